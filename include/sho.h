@@ -1,0 +1,136 @@
+/*
+ * sho.h -- C ABI of libsho: the PAW projection hot path with analytical Spherical-Harmonic-
+ * Oscillator (SHO) projectors on one NVIDIA B200 (sm_100a).
+ *
+ * Method: Baumeister & Tsukamoto, "Analytical PAW Projector Functions for Reduced Bandwidth
+ * Requirements", PASC'19 (arXiv:1905.00480).  Citations are PAPER.md:<line>.
+ *
+ *   projection  (step (1); eq. (25)-(26))
+ *       c[a][b][n(nx,ny,nz)] = h^3 * sum_r psi_b(r) phi_nx(x-X_a) phi_ny(y-Y_a) phi_nz(z-Z_a)
+ *   expansion / add-back  (step (3))
+ *       psi_b(r) += sum_a sum_n c[a][b][n] phi_nx(x-X_a) phi_ny(y-Y_a) phi_nz(z-Z_a)
+ *   with nx+ny+nz <= numax (eq. (17)-(18)) and phi_n the orthonormal 1D
+ *   Hermite-Gauss function of width sigma_a (eq. (3)), sampled ON THE FLY with the
+ *   three-term recurrence of eq. (31), PAPER.md:283-286 -- no projector table is read from memory.
+ *   sho_project_stored is the paper's "USU" baseline: the same projection
+ *   reading pre-sampled 3D projector tables from device memory.
+ *
+ * Conventions:
+ *   - grid point i of axis d sits at x_i = i*h (Bohr); the cell is [0, N_d*h)
+ *   - region of atom a: axis-aligned cube |u_d| <= rcut_sigma*sigma_a, inclusive:
+ *       i_lo = ceil((R_d - rcut_sigma*sigma)/h), i_hi = floor((R_d + rcut_sigma*sigma)/h)
+ *   - periodic axis: indices wrap (j = i mod N); isolated axis: psi == 0 outside, the box is clipped
+ *   - Bloch phase: the value read at image m of axis d is multiplied by exp(2 pi i kfrac[d] m) in
+ *     project and by its conjugate in add (complex dtypes only)
+ *   - coefficient order: n = 0; for nz: for ny: for nx (nx fastest) with nx+ny+nz <= numax
+ *   - layouts: psi [nbands][Nz][Ny][Nx] (x fastest); coeff [natoms][nbands][N_SHO] (n fastest);
+ *     complex data interleaved (re,im) as in C99 / torch.complex128
+ *   - h^3 volume element in project only (so sho_add == adjoint(sho_project) / h^3)
+ *
+ * Ownership / errors: the caller owns every buffer it passes; the library owns only the opaque
+ * handles it returns.  Every function returns a status and never throws or aborts across the
+ * boundary; sho_last_error() gives a thread-local detail string.  The DEVICE-pointer hot calls
+ * (sho_project, sho_add, sho_project_stored) allocate nothing, are asynchronous on the given CUDA
+ * stream and never synchronise the host.  psi must be finite on the whole grid (values just outside
+ * a box are multiplied by exact zeros).  There is no CPU fallback: without a CUDA device every call
+ * that needs one returns SHO_ERR_CUDA.
+ */
+#ifndef SHO_H_
+#define SHO_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SHO_NUMAX_MAX 15   /* nx+ny+nz <= numax <= 15 (N_SHO <= 816) */
+
+typedef enum {
+    SHO_OK = 0,
+    SHO_ERR_INVALID_ARG = 1,  /* null pointer, h <= 0, sigma <= 0, numax out of range, dtype mismatch ... */
+    SHO_ERR_UNSUPPORTED = 2,  /* valid problem the GPU path does not cover (e.g. periodic box wider than the cell) */
+    SHO_ERR_OOM = 3,          /* device allocation failed / tables do not fit */
+    SHO_ERR_CUDA = 4          /* CUDA runtime error, or no device */
+} sho_status;
+
+/* element type of psi and coeff; arithmetic is IEEE double for all four (fp32 data are widened on
+ * load and rounded once on store) */
+typedef enum { SHO_R64 = 0, SHO_C128 = 1, SHO_R32 = 2, SHO_C64 = 3 } sho_dtype;
+
+typedef struct sho_plan sho_plan;     /* opaque, library-owned: geometry of one set of atoms on one grid */
+typedef struct sho_tables sho_tables; /* opaque, library-owned: pre-sampled 3D projector tables          */
+
+/* eq. (18): (numax+1)(numax+2)(numax+3)/6; -1 if numax is outside [0, SHO_NUMAX_MAX] */
+int sho_nsho(int numax);
+/* position of (nx,ny,nz) in a coefficient vector (order above); -1 if not in the basis */
+int sho_index(int nx, int ny, int nz, int numax);
+
+const char* sho_status_string(sho_status s);
+const char* sho_last_error(void);
+
+/*
+ * Build a plan (set-up, not part of the timed hot path): integer box ranges, wrap segments, the
+ * spatially sorted atom order used for L2-friendly scheduling, and the tile -> atom-image lists that
+ * let sho_add own each psi tile instead of using atomics.  Uses the current CUDA device.
+ *   ng        HOST [3] = Nx, Ny, Nz (each >= 1)
+ *   h         grid spacing in Bohr (> 0)
+ *   periodic  HOST [3], 1 = periodic, 0 = isolated
+ *   kfrac     HOST [3] Bloch phase per wrap = exp(2 pi i kfrac[d]); NULL = all zero.  Must be NULL or
+ *             zero for real dtypes.
+ *   natoms    >= 0;  pos HOST [natoms][3] (Bohr, any real value on periodic axes);  sigma HOST [natoms] (> 0)
+ *   numax     0..SHO_NUMAX_MAX;  rcut_sigma > 0 (the configs use 6.0)
+ * Returns SHO_ERR_UNSUPPORTED if a box on a periodic axis is wider than the cell.
+ */
+sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const int32_t periodic[3],
+                           const double kfrac[3], int32_t natoms, const double* pos, const double* sigma,
+                           int32_t numax, double rcut_sigma, sho_dtype dtype);
+sho_status sho_plan_destroy(sho_plan* plan);
+
+/* test hook: integer box ranges, HOST lo_hi[natoms][3][2] = (i_lo, i_hi) per axis (unwrapped) */
+sho_status sho_plan_boxes(const sho_plan* plan, int32_t* lo_hi);
+
+/* sizes: HOST info[8] = { natoms, N_SHO, numax, dtype, sum over atoms of box points, number of
+ * non-empty add tiles, number of (tile, atom-image) pairs, atoms with a non-empty box } */
+sho_status sho_plan_info(const sho_plan* plan, int64_t info[8]);
+
+/*
+ * Projection, on-the-fly SHO.  psi DEVICE [nbands][Nz][Ny][Nx]; coeff DEVICE [natoms][nbands][N_SHO]
+ * (overwritten; atoms with an empty box get zeros).  cuda_stream is a cudaStream_t (NULL = default).
+ */
+sho_status sho_project(const sho_plan* plan, const void* psi, int32_t nbands, void* coeff, void* cuda_stream);
+
+/* Expansion / add-back, on-the-fly SHO: psi += A coeff.  coeff DEVICE (read), psi DEVICE (in/out).
+ * Deterministic: every psi value is accumulated by exactly one thread, atoms in ascending order. */
+sho_status sho_add(const sho_plan* plan, const void* coeff, int32_t nbands, void* psi, void* cuda_stream);
+
+/*
+ * Stored-projector baseline (the paper's "USU" kernels).
+ * sho_tables_build samples Phi_n(r - R_a) over every box into device memory (element type = the
+ * real type of the plan's dtype).  *bytes_needed is always filled; if the tables do not fit in free
+ * device memory the call returns SHO_ERR_OOM and *out = NULL.  Pass out = NULL to query the size only.
+ */
+sho_status sho_tables_build(const sho_plan* plan, sho_tables** out, size_t* bytes_needed, void* cuda_stream);
+sho_status sho_tables_destroy(sho_tables* tables);
+sho_status sho_project_stored(const sho_plan* plan, const sho_tables* tables, const void* psi, int32_t nbands,
+                              void* coeff, void* cuda_stream);
+
+/*
+ * End-to-end variants with HOST buffers (pinned or pageable): copy in, run the same kernels, copy
+ * out, and synchronise the stream before returning.  They use a device workspace owned by the plan
+ * that is grown on demand (the only hot-path calls that may allocate).
+ *   sho_project_host: psi HOST (read), coeff HOST (written)
+ *   sho_add_host:     coeff HOST (read), psi HOST (in/out)
+ */
+sho_status sho_project_host(sho_plan* plan, const void* psi_host, int32_t nbands, void* coeff_host, void* cuda_stream);
+sho_status sho_add_host(sho_plan* plan, const void* coeff_host, int32_t nbands, void* psi_host, void* cuda_stream);
+
+/* FP64 FMA-pipe micro-benchmark used by bench.py for the roofline denominator: runs `iters` rounds of
+ * dependent DMMA chains on every SM and returns the achieved FLOP/s in *flops_per_s (synchronises). */
+sho_status sho_measure_fp64_peak(int32_t iters, double* flops_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SHO_H_ */

@@ -1,0 +1,476 @@
+// sho_api.cu -- the C ABI of libsho (include/sho.h): argument validation, the plan (step a0 of
+// integer box ranges, spatial atom order, tile -> atom-image lists for the ownership-tiled
+// add), the HOST-buffer end-to-end variants and the FP64 micro-benchmark.  All arithmetic of the hot
+// path lives in the kernels (sho_project.cu, sho_add.cu, sho_stored.cu).
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "sho_internal.h"
+
+namespace sho {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+sho_status cuda_fail(cudaError_t e, const char* what)
+{
+    set_error("%s: %s", what, cudaGetErrorString(e));
+    return (e == cudaErrorMemoryAllocation) ? SHO_ERR_OOM : SHO_ERR_CUDA;
+}
+
+static int floordiv_h(int i, int n)
+{
+    int q = i / n;
+    return (i % n < 0) ? q - 1 : q;
+}
+
+template <typename T>
+static sho_status upload(T** dst, const std::vector<T>& src, const char* what)
+{
+    *dst = nullptr;
+    const size_t bytes = sizeof(T) * std::max<size_t>(src.size(), 1);
+    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(dst), bytes);
+    if (e != cudaSuccess) return cuda_fail(e, what);
+    if (!src.empty()) {
+        e = cudaMemcpy(*dst, src.data(), sizeof(T) * src.size(), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) return cuda_fail(e, what);
+    }
+    return SHO_OK;
+}
+
+static void plan_free_device(sho_plan* p)
+{
+    cudaFree(p->d_atoms); cudaFree(p->d_order); cudaFree(p->d_nxyz);
+    cudaFree(p->d_tile_ptr); cudaFree(p->d_tile_ent); cudaFree(p->d_tile_list);
+    cudaFree(p->ws_psi); cudaFree(p->ws_c);
+    p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr;
+    p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr;
+    p->ws_psi = nullptr; p->ws_c = nullptr;
+}
+
+}  // namespace sho
+
+using namespace sho;
+
+extern "C" {
+
+int sho_nsho(int numax)
+{
+    if (numax < 0 || numax > SHO_NUMAX_MAX) return -1;
+    return (numax + 1) * (numax + 2) * (numax + 3) / 6;
+}
+
+// closed form of the enumeration "for nz: for ny: for nx" (reading A8): entries before plane nz, then
+// before row ny inside that plane, then nx
+int sho_index(int nx, int ny, int nz, int numax)
+{
+    if (numax < 0 || numax > SHO_NUMAX_MAX || nx < 0 || ny < 0 || nz < 0 || nx + ny + nz > numax) return -1;
+    int n = 0;
+    for (int kz = 0; kz < nz; ++kz) { const int m = numax - kz + 1; n += m * (m + 1) / 2; }
+    for (int ky = 0; ky < ny; ++ky) n += numax - nz - ky + 1;
+    return n + nx;
+}
+
+const char* sho_status_string(sho_status s)
+{
+    switch (s) {
+        case SHO_OK: return "SHO_OK";
+        case SHO_ERR_INVALID_ARG: return "SHO_ERR_INVALID_ARG";
+        case SHO_ERR_UNSUPPORTED: return "SHO_ERR_UNSUPPORTED";
+        case SHO_ERR_OOM: return "SHO_ERR_OOM";
+        case SHO_ERR_CUDA: return "SHO_ERR_CUDA";
+    }
+    return "SHO_ERR_?";
+}
+
+const char* sho_last_error(void) { return g_err; }
+
+sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const int32_t periodic[3],
+                           const double kfrac[3], int32_t natoms, const double* pos, const double* sigma,
+                           int32_t numax, double rcut_sigma, sho_dtype dtype)
+{
+    if (out) *out = nullptr;
+    if (!out || !ng || !periodic) { set_error("sho_plan_create: null argument"); return SHO_ERR_INVALID_ARG; }
+    if (natoms < 0 || (natoms > 0 && (!pos || !sigma))) { set_error("sho_plan_create: bad natoms / null pos, sigma"); return SHO_ERR_INVALID_ARG; }
+    if (!(h > 0.0) || !std::isfinite(h)) { set_error("sho_plan_create: h must be > 0"); return SHO_ERR_INVALID_ARG; }
+    if (!(rcut_sigma > 0.0) || !std::isfinite(rcut_sigma)) { set_error("sho_plan_create: rcut_sigma must be > 0"); return SHO_ERR_INVALID_ARG; }
+    if (numax < 0 || numax > SHO_NUMAX_MAX) { set_error("sho_plan_create: numax must be in [0, %d]", SHO_NUMAX_MAX); return SHO_ERR_INVALID_ARG; }
+    if (dtype != SHO_R64 && dtype != SHO_C128 && dtype != SHO_R32 && dtype != SHO_C64) { set_error("sho_plan_create: bad dtype"); return SHO_ERR_INVALID_ARG; }
+    for (int d = 0; d < 3; ++d) {
+        if (ng[d] < 1) { set_error("sho_plan_create: grid dims must be >= 1"); return SHO_ERR_INVALID_ARG; }
+        if (kfrac && kfrac[d] != 0.0 && !is_complex(dtype)) { set_error("sho_plan_create: kfrac != 0 needs a complex dtype"); return SHO_ERR_INVALID_ARG; }
+        if (kfrac && !std::isfinite(kfrac[d])) { set_error("sho_plan_create: kfrac not finite"); return SHO_ERR_INVALID_ARG; }
+    }
+    if ((double)ng[0] * ng[1] * ng[2] > 2.0e9) { set_error("sho_plan_create: more than 2e9 grid points per band"); return SHO_ERR_UNSUPPORTED; }
+    for (int a = 0; a < natoms; ++a) {
+        if (!(sigma[a] > 0.0) || !std::isfinite(sigma[a])) { set_error("sho_plan_create: sigma[%d] must be > 0", a); return SHO_ERR_INVALID_ARG; }
+        for (int d = 0; d < 3; ++d)
+            if (!std::isfinite(pos[3 * a + d])) { set_error("sho_plan_create: pos[%d] not finite", a); return SHO_ERR_INVALID_ARG; }
+    }
+
+    sho_plan* p = new (std::nothrow) sho_plan();
+    if (!p) { set_error("sho_plan_create: host allocation failed"); return SHO_ERR_OOM; }
+    p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr;
+    p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr;
+    p->ws_psi = nullptr; p->ws_c = nullptr; p->ws_psi_bytes = 0; p->ws_c_bytes = 0;
+    p->rcut_sigma = rcut_sigma;
+    p->dtype = dtype;
+    std::memset(&p->g, 0, sizeof(p->g));
+    GridDev& g = p->g;
+    for (int d = 0; d < 3; ++d) {
+        g.ng[d] = ng[d];
+        g.periodic[d] = periodic[d] ? 1 : 0;
+        g.kfrac[d] = (kfrac && is_complex(dtype) && periodic[d]) ? kfrac[d] : 0.0;
+    }
+    g.h = h;
+    g.numax = numax;
+    g.nsho = sho_nsho(numax);
+    g.natoms = natoms;
+    g.has_phase = (g.kfrac[0] != 0.0 || g.kfrac[1] != 0.0 || g.kfrac[2] != 0.0) ? 1 : 0;
+    {   // sqrt(2^n / n!): turns the monic recurrence of eq. (31) into the orthonormal functions (reading A1)
+        double r = 1.0;
+        for (int n = 0; n <= SHO_NUMAX_MAX; ++n) {
+            if (n > 0) r *= 2.0 / (double)n;
+            g.hnorm[n] = std::sqrt(r);
+        }
+    }
+
+    // ---- integer box ranges (reading A3/A5), evaluated in IEEE double exactly as written ----
+    p->atoms.resize(natoms);
+    p->max_n[0] = p->max_n[1] = p->max_n[2] = 0;
+    p->sum_box = 0;
+    std::vector<int32_t> nonempty, empty;
+    for (int a = 0; a < natoms; ++a) {
+        AtomDev& at = p->atoms[a];
+        std::memset(&at, 0, sizeof(at));
+        at.sigma = sigma[a];
+        bool is_empty = false;
+        int64_t npts = 1;
+        for (int d = 0; d < 3; ++d) {
+            at.pos[d] = pos[3 * a + d];
+            volatile double r = rcut_sigma * sigma[a];
+            volatile double lo_x = pos[3 * a + d] - r;
+            volatile double hi_x = pos[3 * a + d] + r;
+            const double lo_f = std::ceil(lo_x / h), hi_f = std::floor(hi_x / h);
+            if (std::fabs(lo_f) > 1.0e9 || std::fabs(hi_f) > 1.0e9) {
+                set_error("sho_plan_create: atom %d box index out of the 32-bit range", a);
+                delete p;
+                return SHO_ERR_INVALID_ARG;
+            }
+            int lo = (int)lo_f, hi = (int)hi_f;
+            if (!g.periodic[d]) { lo = std::max(lo, 0); hi = std::min(hi, ng[d] - 1); }
+            else if (hi - lo + 1 > ng[d]) {
+                set_error("sho_plan_create: atom %d: box of %d points is wider than the periodic cell (%d) on axis %d",
+                          a, hi - lo + 1, ng[d], d);
+                delete p;
+                return SHO_ERR_UNSUPPORTED;
+            }
+            at.lo[d] = lo; at.hi[d] = hi;
+            if (hi < lo) is_empty = true;
+            npts *= std::max(hi - lo + 1, 0);
+        }
+        if (is_empty) { empty.push_back(a); continue; }
+        nonempty.push_back(a);
+        p->sum_box += npts;
+        for (int d = 0; d < 3; ++d) p->max_n[d] = std::max(p->max_n[d], at.hi[d] - at.lo[d] + 1);
+    }
+
+    // ---- spatial order: z-slab major, so CTAs that run together read neighbouring psi from L2 ----
+    {
+        auto cell = [&](int a, int d) {
+            const AtomDev& at = p->atoms[a];
+            const int mid = (at.lo[d] + at.hi[d]) / 2;
+            const int j = g.periodic[d] ? mid - floordiv_h(mid, g.ng[d]) * g.ng[d] : mid;
+            return j / 16;
+        };
+        std::stable_sort(nonempty.begin(), nonempty.end(), [&](int a, int b) {
+            const int za = cell(a, 2), zb = cell(b, 2);
+            if (za != zb) return za < zb;
+            const int ya = cell(a, 1), yb = cell(b, 1);
+            if (ya != yb) return ya < yb;
+            return cell(a, 0) < cell(b, 0);
+        });
+    }
+    p->n_nonempty = (int32_t)nonempty.size();
+    p->order = nonempty;
+    p->order.insert(p->order.end(), empty.begin(), empty.end());
+
+    // ---- (nx,ny,nz) of every coefficient, packed (reading A8) ----
+    std::vector<uint32_t> nxyz;
+    for (int nz = 0; nz <= numax; ++nz)
+        for (int ny = 0; ny <= numax - nz; ++ny)
+            for (int nx = 0; nx <= numax - nz - ny; ++nx) nxyz.push_back((uint32_t)nx | ((uint32_t)ny << 8) | ((uint32_t)nz << 16));
+
+    // ---- add tiling: for every psi tile the (atom, image) pairs whose box touches it, atoms ascending ----
+    const int T[3] = { kAddTX, kAddTY, kAddTZ };
+    for (int d = 0; d < 3; ++d) p->ntile[d] = (ng[d] + T[d] - 1) / T[d];
+    p->ntiles = (int64_t)p->ntile[0] * p->ntile[1] * p->ntile[2];
+    std::vector<int32_t> tile_ptr((size_t)p->ntiles + 1, 0);
+    std::vector<AddEntry> tile_ent;
+    {
+        struct AxisHit { int32_t tile, m; };
+        auto axis_hits = [&](const AtomDev& at, int d, std::vector<AxisHit>& hits) {
+            hits.clear();
+            const int N = g.ng[d];
+            const int m0 = g.periodic[d] ? floordiv_h(at.lo[d], N) : 0;
+            const int m1 = g.periodic[d] ? floordiv_h(at.hi[d], N) : 0;
+            for (int m = m0; m <= m1; ++m)
+                for (int t = 0; t < p->ntile[d]; ++t) {
+                    const int a0 = t * T[d] + m * N, a1 = std::min((t + 1) * T[d], N) - 1 + m * N;
+                    if (a1 >= at.lo[d] && a0 <= at.hi[d]) hits.push_back({ t, m });
+                }
+        };
+        std::vector<AxisHit> hx, hy, hz;
+        for (int pass = 0; pass < 2; ++pass) {
+            std::vector<int32_t> fill;
+            if (pass == 1) {
+                int64_t run = 0;
+                for (int64_t t = 0; t < p->ntiles; ++t) { const int32_t c = tile_ptr[t + 1]; tile_ptr[t] = (int32_t)run; run += c; }
+                // tile_ptr[t] now = start of tile t; counts were stored at [t+1]
+                if (run > 0x7fffffffLL) { set_error("sho_plan_create: too many (tile, atom) pairs"); delete p; return SHO_ERR_UNSUPPORTED; }
+                tile_ptr[p->ntiles] = (int32_t)run;
+                tile_ent.resize((size_t)run);
+                fill.assign(tile_ptr.begin(), tile_ptr.end() - 1);
+            }
+            for (int a = 0; a < natoms; ++a) {
+                const AtomDev& at = p->atoms[a];
+                if (at.hi[0] < at.lo[0] || at.hi[1] < at.lo[1] || at.hi[2] < at.lo[2]) continue;
+                axis_hits(at, 0, hx); axis_hits(at, 1, hy); axis_hits(at, 2, hz);
+                for (const AxisHit& z : hz)
+                    for (const AxisHit& y : hy)
+                        for (const AxisHit& x : hx) {
+                            const int64_t t = ((int64_t)z.tile * p->ntile[1] + y.tile) * p->ntile[0] + x.tile;
+                            if (pass == 0) tile_ptr[t + 1] += 1;
+                            else {
+                                AddEntry e; e.atom = a; e.m[0] = x.m; e.m[1] = y.m; e.m[2] = z.m;
+                                tile_ent[(size_t)fill[t]++] = e;
+                            }
+                        }
+            }
+            if (pass == 0 && p->ntiles > 0) {
+                // keep counts at [t+1]; the prefix sum happens at the start of pass 1
+            }
+        }
+    }
+    p->npairs = (int64_t)tile_ent.size();
+    std::vector<int32_t> tile_list;
+    for (int64_t t = 0; t < p->ntiles; ++t)
+        if (tile_ptr[t + 1] > tile_ptr[t]) tile_list.push_back((int32_t)t);
+    p->n_tile_list = (int32_t)tile_list.size();
+
+    // ---- device mirrors ----
+    cudaError_t e = cudaGetDevice(&p->device);
+    if (e != cudaSuccess) { sho_status s = cuda_fail(e, "sho_plan_create: cudaGetDevice (no CUDA device?)"); delete p; return s; }
+    sho_status st;
+    if ((st = upload(&p->d_atoms, p->atoms, "sho_plan_create: atoms")) != SHO_OK ||
+        (st = upload(&p->d_order, p->order, "sho_plan_create: order")) != SHO_OK ||
+        (st = upload(&p->d_nxyz, nxyz, "sho_plan_create: nxyz")) != SHO_OK ||
+        (st = upload(&p->d_tile_ptr, tile_ptr, "sho_plan_create: tile_ptr")) != SHO_OK ||
+        (st = upload(&p->d_tile_ent, tile_ent, "sho_plan_create: tile_ent")) != SHO_OK ||
+        (st = upload(&p->d_tile_list, tile_list, "sho_plan_create: tile_list")) != SHO_OK) {
+        plan_free_device(p);
+        delete p;
+        return st;
+    }
+    *out = p;
+    return SHO_OK;
+}
+
+sho_status sho_plan_destroy(sho_plan* plan)
+{
+    if (!plan) return SHO_OK;
+    plan_free_device(plan);
+    delete plan;
+    return SHO_OK;
+}
+
+sho_status sho_plan_boxes(const sho_plan* plan, int32_t* lo_hi)
+{
+    if (!plan || !lo_hi) { set_error("sho_plan_boxes: null argument"); return SHO_ERR_INVALID_ARG; }
+    for (size_t a = 0; a < plan->atoms.size(); ++a)
+        for (int d = 0; d < 3; ++d) {
+            lo_hi[(a * 3 + d) * 2 + 0] = plan->atoms[a].lo[d];
+            lo_hi[(a * 3 + d) * 2 + 1] = plan->atoms[a].hi[d];
+        }
+    return SHO_OK;
+}
+
+sho_status sho_plan_info(const sho_plan* plan, int64_t info[8])
+{
+    if (!plan || !info) { set_error("sho_plan_info: null argument"); return SHO_ERR_INVALID_ARG; }
+    info[0] = plan->g.natoms; info[1] = plan->g.nsho; info[2] = plan->g.numax; info[3] = (int64_t)plan->dtype;
+    info[4] = plan->sum_box; info[5] = plan->n_tile_list; info[6] = plan->npairs; info[7] = plan->n_nonempty;
+    return SHO_OK;
+}
+
+static sho_status check_hot(const char* fn, const sho_plan* plan, const void* a, const void* b, int32_t nbands)
+{
+    if (!plan || !a || !b) { set_error("%s: null argument", fn); return SHO_ERR_INVALID_ARG; }
+    if (nbands <= 0) { set_error("%s: nbands must be > 0", fn); return SHO_ERR_INVALID_ARG; }
+    return SHO_OK;
+}
+
+sho_status sho_project(const sho_plan* plan, const void* psi, int32_t nbands, void* coeff, void* cuda_stream)
+{
+    if (plan && plan->g.natoms == 0 && psi && nbands > 0) return SHO_OK;   // coeff is empty (may be null)
+    sho_status st = check_hot("sho_project", plan, psi, coeff, nbands);
+    if (st != SHO_OK) return st;
+    return launch_project(plan, psi, nbands, coeff, static_cast<cudaStream_t>(cuda_stream));
+}
+
+sho_status sho_add(const sho_plan* plan, const void* coeff, int32_t nbands, void* psi, void* cuda_stream)
+{
+    if (plan && plan->g.natoms == 0 && psi && nbands > 0) return SHO_OK;   // coeff is empty (may be null)
+    sho_status st = check_hot("sho_add", plan, coeff, psi, nbands);
+    if (st != SHO_OK) return st;
+    if (plan->n_tile_list == 0) return SHO_OK;
+    return launch_add(plan, coeff, nbands, psi, static_cast<cudaStream_t>(cuda_stream));
+}
+
+sho_status sho_tables_build(const sho_plan* plan, sho_tables** out, size_t* bytes_needed, void* cuda_stream)
+{
+    if (out) *out = nullptr;
+    if (!plan || !bytes_needed) { set_error("sho_tables_build: null argument"); return SHO_ERR_INVALID_ARG; }
+    return tables_build(plan, out, bytes_needed, static_cast<cudaStream_t>(cuda_stream));
+}
+
+sho_status sho_tables_destroy(sho_tables* t)
+{
+    if (!t) return SHO_OK;
+    cudaFree(t->d_data);
+    cudaFree(t->d_atom_off);
+    cudaFree(t->d_seg_atom);
+    cudaFree(t->d_seg_qz0);
+    delete t;
+    return SHO_OK;
+}
+
+sho_status sho_project_stored(const sho_plan* plan, const sho_tables* tables, const void* psi, int32_t nbands,
+                              void* coeff, void* cuda_stream)
+{
+    if (plan && plan->g.natoms == 0 && psi && nbands > 0 && tables && tables->plan == plan) return SHO_OK;
+    sho_status st = check_hot("sho_project_stored", plan, psi, coeff, nbands);
+    if (st != SHO_OK) return st;
+    if (!tables || tables->plan != plan) { set_error("sho_project_stored: tables do not belong to this plan"); return SHO_ERR_INVALID_ARG; }
+    return launch_project_stored(plan, tables, psi, nbands, coeff, static_cast<cudaStream_t>(cuda_stream));
+}
+
+// ---- HOST-buffer end-to-end variants ------------------------------------------------------------
+static sho_status ws_reserve(void** ws, size_t* have, size_t need, const char* what)
+{
+    if (*have >= need) return SHO_OK;
+    cudaFree(*ws);
+    *ws = nullptr; *have = 0;
+    cudaError_t e = cudaMalloc(ws, need);
+    if (e != cudaSuccess) { cudaGetLastError(); set_error("%s: cannot allocate %zu bytes of device workspace", what, need); return SHO_ERR_OOM; }
+    *have = need;
+    return SHO_OK;
+}
+
+sho_status sho_project_host(sho_plan* plan, const void* psi_host, int32_t nbands, void* coeff_host, void* cuda_stream)
+{
+    sho_status st = check_hot("sho_project_host", plan, psi_host, coeff_host, nbands);
+    if (st != SHO_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const size_t esz = elem_size(plan->dtype);
+    const size_t psi_bytes = (size_t)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * nbands * esz;
+    const size_t c_bytes = (size_t)plan->g.natoms * nbands * plan->g.nsho * esz;
+    if ((st = ws_reserve(&plan->ws_psi, &plan->ws_psi_bytes, psi_bytes, "sho_project_host")) != SHO_OK) return st;
+    if ((st = ws_reserve(&plan->ws_c, &plan->ws_c_bytes, std::max<size_t>(c_bytes, 16), "sho_project_host")) != SHO_OK) return st;
+    cudaError_t e = cudaMemcpyAsync(plan->ws_psi, psi_host, psi_bytes, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(e, "sho_project_host: H2D psi");
+    if (plan->g.natoms > 0) {
+        if ((st = launch_project(plan, plan->ws_psi, nbands, plan->ws_c, s)) != SHO_OK) return st;
+        e = cudaMemcpyAsync(coeff_host, plan->ws_c, c_bytes, cudaMemcpyDeviceToHost, s);
+        if (e != cudaSuccess) return cuda_fail(e, "sho_project_host: D2H coeff");
+    }
+    e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(e, "sho_project_host: synchronize");
+    return SHO_OK;
+}
+
+sho_status sho_add_host(sho_plan* plan, const void* coeff_host, int32_t nbands, void* psi_host, void* cuda_stream)
+{
+    sho_status st = check_hot("sho_add_host", plan, coeff_host, psi_host, nbands);
+    if (st != SHO_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const size_t esz = elem_size(plan->dtype);
+    const size_t psi_bytes = (size_t)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * nbands * esz;
+    const size_t c_bytes = (size_t)plan->g.natoms * nbands * plan->g.nsho * esz;
+    if (plan->g.natoms == 0 || plan->n_tile_list == 0) return SHO_OK;
+    if ((st = ws_reserve(&plan->ws_psi, &plan->ws_psi_bytes, psi_bytes, "sho_add_host")) != SHO_OK) return st;
+    if ((st = ws_reserve(&plan->ws_c, &plan->ws_c_bytes, std::max<size_t>(c_bytes, 16), "sho_add_host")) != SHO_OK) return st;
+    cudaError_t e = cudaMemcpyAsync(plan->ws_psi, psi_host, psi_bytes, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: H2D psi");
+    e = cudaMemcpyAsync(plan->ws_c, coeff_host, c_bytes, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: H2D coeff");
+    if ((st = launch_add(plan, plan->ws_c, nbands, plan->ws_psi, s)) != SHO_OK) return st;
+    e = cudaMemcpyAsync(psi_host, plan->ws_psi, psi_bytes, cudaMemcpyDeviceToHost, s);
+    if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: D2H psi");
+    e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: synchronize");
+    return SHO_OK;
+}
+
+}  // extern "C"
+
+// ---- FP64 pipe micro-benchmark (roofline denominator measured in the same run) ------------------
+namespace sho {
+__global__ void __launch_bounds__(512) fp64_peak_kernel(double* out, int iters, double s)
+{
+    double a[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = threadIdx.x * 1e-3 + i;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) a[i] = fma(a[i], s, s);
+    }
+    double r = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) r += a[i];
+    if (r == 12345.678) out[0] = r;   // never true; keeps the chain alive
+}
+}  // namespace sho
+
+extern "C" sho_status sho_measure_fp64_peak(int32_t iters, double* flops_per_s)
+{
+    if (!flops_per_s || iters <= 0) { set_error("sho_measure_fp64_peak: bad argument"); return SHO_ERR_INVALID_ARG; }
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "sho_measure_fp64_peak: cudaGetDevice");
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    double* d = nullptr;
+    if ((e = cudaMalloc(&d, 8)) != cudaSuccess) return cuda_fail(e, "sho_measure_fp64_peak: cudaMalloc");
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = 2 * sms, threads = 512;
+    sho::fp64_peak_kernel<<<blocks, threads>>>(d, iters, 0.999);   // warm-up
+    double best = 0.0;
+    for (int rep = 0; rep < 3; ++rep) {
+        cudaEventRecord(e0);
+        sho::fp64_peak_kernel<<<blocks, threads>>>(d, iters, 0.999);
+        cudaEventRecord(e1);
+        e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double fl = 2.0 * 8.0 * (double)iters * blocks * threads / (ms * 1e-3);
+        best = std::max(best, fl);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(d);
+    if (e != cudaSuccess) return cuda_fail(e, "sho_measure_fp64_peak");
+    *flops_per_s = best;
+    return SHO_OK;
+}

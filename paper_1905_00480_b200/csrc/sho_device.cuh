@@ -1,0 +1,88 @@
+// sho_device.cuh -- device helpers: the on-the-fly 1D Hermite-Gauss sampler (eq. (31)),
+// the FP64 tensor-core MMA wrapper, typed loads/stores.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "sho_internal.h"
+
+namespace sho {
+
+// D(8x8) += A(8x4) * B(4x8), FP64 tensor core (SASS: DMMA.8x8x4).  Fragment layout, lane = 4*q + t:
+//   a = A[row q][col t],  b = B[row t][col q],  d0,d1 = D[row q][col 2t, 2t+1]
+__device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(d0), "+d"(d1)
+                 : "d"(a), "d"(b));
+}
+
+__device__ __forceinline__ int floordiv(int i, int n)
+{
+    int q = i / n;
+    return (i % n < 0) ? q - 1 : q;
+}
+
+// Orthonormal Hermite-Gauss functions phi_0..phi_{NMAX-1} of width sigma at displacement u (step a1):
+// the paper's monic three-term recurrence, eq. (31) PAPER.md:283-284,
+//     H_0 = 1, H_1 = xi, H_{n+1} = xi H_n - (n/2) H_{n-1},
+// times the Gaussian of eq. (3) PAPER.md:70 and the normalisation the paper leaves to the D matrices
+// (PAPER.md:286): phi_n = sqrt(2^n/n!) (sqrt(pi) sigma)^(-1/2) H_n(xi) exp(-xi^2/2), xi = u/sigma.
+// Entries with n > numax (or valid == false) are written as exact zeros.
+template <int NMAX>
+__device__ __forceinline__ void hermite_gauss(double u, double sigma, const double* __restrict__ hnorm, int numax,
+                                              bool valid, double (&out)[NMAX])
+{
+    const double xi = u / sigma;
+    const double g = valid ? exp(-0.5 * xi * xi) * rsqrt(1.7724538509055160273 * sigma) : 0.0;
+    double hm = 0.0, hc = 1.0;
+#pragma unroll
+    for (int n = 0; n < NMAX; ++n) {
+        out[n] = (n <= numax) ? hc * g * hnorm[n < SHO_NUMAX_MAX ? n : SHO_NUMAX_MAX] : 0.0;
+        const double hn = xi * hc - (0.5 * (double)n) * hm;
+        hm = hc;
+        hc = hn;
+    }
+}
+
+// unwrapped index -> displacement from the atom, written as the paper's grid convention x_i = i*h
+// (no FMA contraction, so box-edge values match a plain evaluation)
+__device__ __forceinline__ double displacement(int i, double h, double pos) { return __dsub_rn(__dmul_rn((double)i, h), pos); }
+
+// ---- typed access: element type -> two fp64 lanes per 16/8-byte load -------------------------------
+template <int DT> struct Elem;
+template <> struct Elem<SHO_R64>  { using real_t = double; static constexpr bool cplx = false; static constexpr int cw = 16; };
+template <> struct Elem<SHO_R32>  { using real_t = float;  static constexpr bool cplx = false; static constexpr int cw = 16; };
+template <> struct Elem<SHO_C128> { using real_t = double; static constexpr bool cplx = true;  static constexpr int cw = 8; };
+template <> struct Elem<SHO_C64>  { using real_t = float;  static constexpr bool cplx = true;  static constexpr int cw = 8; };
+
+__device__ __forceinline__ void load2(const double* p, bool vec, double& v0, double& v1)
+{
+    if (vec) { const double2 v = __ldg(reinterpret_cast<const double2*>(p)); v0 = v.x; v1 = v.y; }
+    else { v0 = __ldg(p); v1 = __ldg(p + 1); }
+}
+__device__ __forceinline__ void load2(const float* p, bool vec, double& v0, double& v1)
+{
+    if (vec) { const float2 v = __ldg(reinterpret_cast<const float2*>(p)); v0 = (double)v.x; v1 = (double)v.y; }
+    else { v0 = (double)__ldg(p); v1 = (double)__ldg(p + 1); }
+}
+
+// plain (coherent) two-element load and store for the read-modify-write of sho_add; p is 2-element aligned
+__device__ __forceinline__ void load2_rw(const double* p, double& v0, double& v1)
+{
+    const double2 v = *reinterpret_cast<const double2*>(p); v0 = v.x; v1 = v.y;
+}
+__device__ __forceinline__ void load2_rw(const float* p, double& v0, double& v1)
+{
+    const float2 v = *reinterpret_cast<const float2*>(p); v0 = (double)v.x; v1 = (double)v.y;
+}
+__device__ __forceinline__ void store2(double* p, double v0, double v1)
+{
+    double2 v; v.x = v0; v.y = v1; *reinterpret_cast<double2*>(p) = v;
+}
+__device__ __forceinline__ void store2(float* p, double v0, double v1)
+{
+    float2 v; v.x = (float)v0; v.y = (float)v1; *reinterpret_cast<float2*>(p) = v;
+}
+
+}  // namespace sho

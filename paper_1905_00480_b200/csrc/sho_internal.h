@@ -1,0 +1,98 @@
+// sho_internal.h -- host-side plan object and kernel parameter blocks shared by the .cu files of
+// libsho.  Not part of the ABI (include/sho.h is).  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/sho.h"
+
+namespace sho {
+
+constexpr int kProjWarps = 8;          // warps per CTA in the project kernel (one z-plane each per round)
+constexpr int kAddTX = 32, kAddTY = 64, kAddTZ = 2;   // psi tile owned by one CTA of the add kernel
+constexpr int kAddWarps = (kAddTX / 8) * kAddTZ;      // one (z, x-block) per warp
+
+// one atom as the kernels see it (64 bytes)
+struct AtomDev {
+    double pos[3];
+    double sigma;
+    int32_t lo[3];   // unwrapped inclusive box range per axis (reading A3); lo > hi on any axis: empty
+    int32_t hi[3];
+    int32_t pad[2];
+};
+
+// one (atom image) that overlaps an add tile: unwrapped index i = j + m*N on each axis
+struct AddEntry {
+    int32_t atom;
+    int32_t m[3];
+};
+
+struct GridDev {
+    int32_t ng[3];
+    int32_t periodic[3];
+    double h;
+    double kfrac[3];
+    double hnorm[SHO_NUMAX_MAX + 1];   // sqrt(2^n / n!): scale of the monic recurrence of eq. (31)
+    int32_t numax;
+    int32_t nsho;
+    int32_t natoms;
+    int32_t has_phase;                 // complex dtype and some kfrac != 0 on a periodic axis
+};
+
+}  // namespace sho
+
+struct sho_plan {
+    sho::GridDev g;
+    double rcut_sigma;
+    sho_dtype dtype;
+    int device;
+    std::vector<sho::AtomDev> atoms;       // host copy, original order
+    std::vector<int32_t> order;            // spatially sorted atom indices (non-empty boxes first)
+    int32_t n_nonempty;
+    int32_t max_n[3];                      // largest box extent per axis
+    int64_t sum_box;                       // sum over atoms of box points
+    // device mirrors
+    sho::AtomDev* d_atoms;
+    int32_t* d_order;
+    uint32_t* d_nxyz;                      // [nsho] packed nx | ny<<8 | nz<<16
+    // add tiling
+    int32_t ntile[3];
+    int64_t ntiles;
+    int64_t npairs;
+    int32_t* d_tile_ptr;                   // [ntiles+1]
+    sho::AddEntry* d_tile_ent;             // [npairs]
+    int32_t* d_tile_list;                  // tiles with at least one entry
+    int32_t n_tile_list;
+    // workspace for the *_host calls
+    void* ws_psi; size_t ws_psi_bytes;
+    void* ws_c;   size_t ws_c_bytes;
+};
+
+struct sho_tables {
+    const sho_plan* plan;
+    void* d_data;                          // fragment-ordered tables, see sho_stored.cu
+    int64_t* d_atom_off;                   // [natoms+1] offsets in elements
+    int32_t* d_seg_atom;                   // K segments (atom, first box plane) = the CTAs of the stored kernel
+    int32_t* d_seg_qz0;
+    int32_t nseg;
+    std::vector<int64_t> atom_off;
+    size_t bytes;
+};
+
+namespace sho {
+
+void set_error(const char* fmt, ...);
+sho_status cuda_fail(cudaError_t e, const char* what);
+inline size_t elem_size(sho_dtype t) { return t == SHO_R64 ? 8 : t == SHO_C128 ? 16 : t == SHO_R32 ? 4 : 8; }
+inline bool is_complex(sho_dtype t) { return t == SHO_C128 || t == SHO_C64; }
+
+// launchers (defined next to their kernels)
+sho_status launch_project(const sho_plan* p, const void* psi, int nbands, void* coeff, cudaStream_t s);
+sho_status launch_add(const sho_plan* p, const void* coeff, int nbands, void* psi, cudaStream_t s);
+sho_status launch_project_stored(const sho_plan* p, const sho_tables* t, const void* psi, int nbands, void* coeff,
+                                 cudaStream_t s);
+sho_status tables_build(const sho_plan* p, sho_tables** out, size_t* bytes_needed, cudaStream_t s);
+
+}  // namespace sho

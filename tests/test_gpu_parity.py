@@ -1,0 +1,270 @@
+"""GPU parity: the CUDA path (through the C ABI of libsho.so) against the CPU oracle, element by element,
+on the same seeded inputs (paper_1905_00480_b200.workloads).  Run with ``-m gpu`` on a B200.
+
+Tolerances (north_star / reading A13):
+  project: max_b max_{a,n} |c_gpu - c_ref| / ||psi_b||      <= 1e-12 (fp64), 1e-5 (fp32),
+           ||psi_b|| = sqrt(h^3 sum_r |psi_b(r)|^2)
+  add:     max_b max_r |psi_gpu - psi_ref| / max_r |psi_ref,b| <= 1e-12 (fp64), 1e-5 (fp32)
+Integer work (box ranges, index map) must agree exactly.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1905_00480_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"r64": 1e-12, "c128": 1e-12, "r32": 1e-5, "c64": 1e-5}
+NP_OF = {"r64": np.float64, "c128": np.complex128, "r32": np.float32, "c64": np.complex64}
+
+
+@pytest.fixture(scope="module")
+def sho():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device")
+    import paper_1905_00480_b200 as pkg
+    pkg.lib()          # raises if libsho.so cannot be loaded: no silent fallback
+    return pkg
+
+
+def _dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _psi_norm(psi, h):
+    return np.sqrt(h ** 3 * np.sum(np.abs(psi.astype(np.complex128 if np.iscomplexobj(psi) else np.float64)) ** 2,
+                                   axis=(1, 2, 3)))
+
+
+def _oracle_boxes(w):
+    out = np.zeros((w.natoms, 3, 2), np.int32)
+    for a in range(w.natoms):
+        lo, hi, _ = oracle.box(w.ng, w.h, w.periodic, w.pos[a], w.sigma[a], w.rcut_sigma)
+        out[a, :, 0], out[a, :, 1] = lo, hi
+    return out
+
+
+def check_project(sho, w, psi, coeff_gpu, tol, pairs=None):
+    """Compare coeff_gpu [na][nb][nsho] (numpy) with the oracle (all pairs, or the listed (a,b) pairs)."""
+    wide = np.complex128 if w.is_complex else np.float64
+    norm = _psi_norm(psi, w.h)
+    if pairs is None:
+        ref = oracle.project(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax, psi.astype(wide), w.rcut_sigma)
+        err = np.abs(coeff_gpu.astype(wide) - ref) / np.maximum(norm, 1e-300)[None, :, None]
+    else:
+        pa, pb = np.array([p[0] for p in pairs]), np.array([p[1] for p in pairs])
+        bands = {int(b): psi[int(b)].astype(wide) for b in np.unique(pb)}
+        ref = oracle.project_pairs(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax, bands, pa, pb,
+                                   psi.shape[0], w.is_complex, w.rcut_sigma)
+        err = np.abs(coeff_gpu[pa, pb].astype(wide) - ref) / norm[pb][:, None]
+    assert np.all(np.isfinite(coeff_gpu))
+    assert err.max() <= tol, "project parity: max normalised error %.3e > %.1e" % (err.max(), tol)
+    return float(err.max())
+
+
+def run_case(sho, w, stored=True, tol=None):
+    """boxes, project, add, stored project of one workload against the oracle (full comparison)."""
+    import torch
+    tol = tol or TOL[w.dtype]
+    wide = np.complex128 if w.is_complex else np.float64
+    plan = sho.plan_for(w)
+    try:
+        assert np.array_equal(plan.boxes(), _oracle_boxes(w)), "integer box ranges differ from the oracle"
+        assert plan.nsho == oracle.nsho(w.numax)
+        psi = w.psi()
+        if w.psi_dist == "zero":     # cfg 4 has psi_0 = 0; project needs something to project
+            psi = workloads.Workload(**{**w.__dict__, "psi_dist": "normal"}).psi()
+        d_psi = _dev(psi)
+        # ---- project ----
+        c_gpu = plan.project(d_psi)
+        torch.cuda.synchronize()
+        e_prj = check_project(sho, w, psi, c_gpu.cpu().numpy(), tol)
+        # ---- stored-projector baseline ----
+        if stored:
+            tb = plan.tables()
+            c_sto = plan.project_stored(tb, d_psi)
+            torch.cuda.synchronize()
+            check_project(sho, w, psi, c_sto.cpu().numpy(), tol)
+            tb.close()
+        # ---- add ----
+        coeff = w.coeff(plan.nsho)
+        psi0 = w.psi()
+        d_psi0 = _dev(psi0)
+        plan.add(_dev(coeff), d_psi0)
+        torch.cuda.synchronize()
+        got = d_psi0.cpu().numpy()
+        ref = oracle.add(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax, coeff.astype(wide), psi0.astype(wide),
+                         w.rcut_sigma)
+        scale = np.maximum(np.abs(ref).max(axis=(1, 2, 3)), 1e-300)
+        err = (np.abs(got.astype(wide) - ref).max(axis=(1, 2, 3)) / scale).max()
+        assert err <= tol, "add parity: max normalised error %.3e > %.1e" % (err, tol)
+        return e_prj, float(err)
+    finally:
+        plan.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# configs at sizes the oracle finishes in seconds
+
+
+def test_cfg1_full_single_atom_isolated(sho):
+    e = run_case(sho, workloads.make(1))
+    assert e[0] < 1e-13 and e[1] < 1e-13        # the contract is loose by orders of magnitude
+
+
+@pytest.mark.parametrize("dtype", ["r32", "c128", "c64"])
+def test_cfg1_other_dtypes(sho, dtype):
+    run_case(sho, workloads.make(1, dtype=dtype))
+
+
+@pytest.mark.parametrize("k", [2, 3, 4, 5])
+def test_small_configs_native_dtype(sho, k):
+    run_case(sho, workloads.make(k, size="small"))
+
+
+@pytest.mark.parametrize("k,dtype", [(4, "r32"), (5, "c64"), (2, "c128"), (3, "r32")])
+def test_small_configs_other_dtypes(sho, k, dtype):
+    w = workloads.make(k, size="small", dtype=dtype)
+    if dtype in ("r32", "r64"):
+        w.kfrac = None
+    run_case(sho, w)
+
+
+# ------------------------------------------------------------------------------------------------
+# edge cases
+
+
+def _custom(ng, periodic, pos, sigma, numax, nb, dtype="r64", h=0.25, kfrac=None, seed=7, rc=6.0):
+    return workloads.Workload("custom", seed, tuple(ng), h, tuple(periodic), kfrac, np.asarray(pos, float).reshape(-1, 3),
+                              np.asarray(sigma, float).reshape(-1), numax, nb, dtype, "normal", rcut_sigma=rc)
+
+
+def test_no_atoms(sho):
+    import torch
+    w = _custom((16, 16, 16), (1, 1, 1), np.zeros((0, 3)), np.zeros(0), 3, 2)
+    plan = sho.plan_for(w)
+    psi = _dev(w.psi())
+    before = psi.clone()
+    c = plan.project(psi)
+    assert tuple(c.shape) == (0, 2, 20)
+    plan.add(c, psi)
+    torch.cuda.synchronize()
+    assert torch.equal(psi, before)
+    plan.close()
+
+
+def test_atoms_outside_and_straddling_an_isolated_grid(sho):
+    # atom 0 far outside (empty box => exact zeros), atom 1 straddles a corner, atom 2 inside
+    pos = [[-30.0, 2.0, 2.0], [0.1, 5.9, 0.3], [3.0, 3.1, 2.9]]
+    w = _custom((24, 28, 20), (0, 0, 0), pos, [0.5, 0.45, 0.4], 4, 3)
+    import torch
+    plan = sho.plan_for(w)
+    c = plan.project(_dev(w.psi()))
+    torch.cuda.synchronize()
+    assert torch.count_nonzero(c[0]) == 0
+    plan.close()
+    run_case(sho, w)
+
+
+@pytest.mark.parametrize("periodic", [(1, 1, 1), (1, 0, 1), (0, 1, 0)])
+def test_odd_ragged_grid_dims(sho, periodic):
+    # Nx odd: the vector loads fall back to scalar; tiles of the add kernel are ragged on every axis
+    rng = np.random.default_rng(11)
+    ng = (33, 37, 29)
+    pos = rng.uniform(0, 1, (5, 3)) * np.array(ng) * 0.25
+    run_case(sho, _custom(ng, periodic, pos, rng.uniform(0.35, 0.6, 5), 5, 2))
+
+
+@pytest.mark.parametrize("numax", [0, 1, 2, 3, 4, 6, 8, 9, 11, 12, 15])
+def test_every_numax_tile_shape(sho, numax):
+    rng = np.random.default_rng(100 + numax)
+    ng = (20, 24, 18)
+    pos = rng.uniform(0, 1, (2, 3)) * np.array(ng) * 0.3
+    # small sigma and a 4-sigma cut keep the box (9-10 points) inside the cell; parity does not need a wide cut
+    run_case(sho, _custom(ng, (1, 1, 1), pos, [0.3, 0.36], numax, 2, h=0.3, rc=4.0), stored=numax <= 9)
+
+
+def test_box_exactly_as_wide_as_the_cell(sho):
+    # periodic box of exactly N points on x (every grid point once, one wrap)
+    ng = (24, 40, 40)
+    w = _custom(ng, (1, 1, 1), [[1.13, 5.0, 5.0]], [0.4834], 3, 2, h=0.25)
+    lo, hi, _ = oracle.box(w.ng, w.h, w.periodic, w.pos[0], w.sigma[0], 6.0)
+    assert hi[0] - lo[0] + 1 == 24
+    run_case(sho, w)
+
+
+def test_box_wider_than_cell_is_reported_unsupported(sho):
+    w = _custom((16, 16, 16), (1, 1, 1), [[1.0, 1.0, 1.0]], [1.0], 2, 1)
+    with pytest.raises(sho.ShoError) as ei:
+        sho.plan_for(w)
+    assert ei.value.status == 2
+
+
+def test_unaligned_psi_pointer(sho):
+    # psi starting 8 bytes into an allocation: the 16-byte vector path must not be taken
+    import torch
+    w = workloads.make(2, size="small")
+    plan = sho.plan_for(w)
+    psi = w.psi()
+    buf = torch.zeros(psi.size + 1, dtype=torch.float64, device="cuda")
+    view = buf[1:].view(psi.shape)
+    view.copy_(torch.from_numpy(psi))
+    c = plan.project(view)
+    torch.cuda.synchronize()
+    check_project(sho, w, psi, c.cpu().numpy(), 1e-12)
+    coeff = w.coeff(plan.nsho)
+    plan.add(_dev(coeff), view)
+    torch.cuda.synchronize()
+    ref = oracle.add(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax, coeff, psi)
+    assert np.abs(view.cpu().numpy() - ref).max() <= 1e-12 * np.abs(ref).max()
+    plan.close()
+
+
+def test_add_is_bit_reproducible(sho):
+    import torch
+    w = workloads.make(4, size="small")
+    plan = sho.plan_for(w)
+    c = _dev(w.coeff(plan.nsho))
+    outs = []
+    for _ in range(3):
+        psi = torch.zeros((w.nbands, w.ng[2], w.ng[1], w.ng[0]), dtype=torch.float64, device="cuda")
+        plan.add(c, psi)
+        torch.cuda.synchronize()
+        outs.append(psi)
+    assert torch.equal(outs[0], outs[1]) and torch.equal(outs[0], outs[2])
+    plan.close()
+
+
+def test_host_buffer_entry_points(sho):
+    w = workloads.make(3, size="small")
+    plan = sho.plan_for(w)
+    psi = w.psi()
+    c = np.zeros((w.natoms, w.nbands, plan.nsho))
+    plan.project_host(psi, c)
+    check_project(sho, w, psi, c, 1e-12)
+    coeff = w.coeff(plan.nsho)
+    out = psi.copy()
+    plan.add_host(coeff, out)
+    ref = oracle.add(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax, coeff, psi)
+    assert np.abs(out - ref).max() <= 1e-12 * np.abs(ref).max()
+    plan.close()
+
+
+def test_wrong_arguments_raise(sho):
+    import torch
+    w = workloads.make(1)
+    plan = sho.plan_for(w)
+    with pytest.raises(ValueError):
+        plan.project(torch.zeros((1, 32, 32, 32), dtype=torch.float32, device="cuda"))
+    with pytest.raises(ValueError):
+        plan.project(torch.zeros((1, 32, 32, 31), dtype=torch.float64, device="cuda"))
+    with pytest.raises(sho.ShoError):
+        sho.Plan((32, 32, 32), -1.0, (0, 0, 0), w.pos, w.sigma, 3)
+    with pytest.raises(sho.ShoError):
+        sho.Plan((32, 32, 32), 0.25, (0, 0, 0), w.pos, w.sigma, 16)
+    with pytest.raises(sho.ShoError):
+        sho.Plan((32, 32, 32), 0.25, (1, 1, 1), w.pos, w.sigma, 3, "r64", kfrac=(0.1, 0, 0))
+    plan.close()
