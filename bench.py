@@ -1,0 +1,332 @@
+#!/usr/bin/env python
+"""bench.py -- SHO project + add-back throughput on B200 (BASELINE.json metric), one JSON line.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+A step is one pass of the whole hot path over one batch of synthetic input: c = sho_project(psi)
+followed by psi' += sho_add(c).  ``value`` is psi-GB/s(box): the bytes of every atom's psi box
+(read once by project, read + written once by add: 3 * sum_a |box_a| * nbands * sizeof(elem)) divided
+by the device time of the step, inputs resident in HBM.  ``e2e`` is the same metric through the
+HOST-buffer C-ABI calls (sho_project_host / sho_add_host), copies inside the timed region.
+``--impl reference`` times the CPU oracle (oracle/, test infrastructure) on a bounded sample.
+See DESIGN.md "Measurement" for every definition used here.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1905_00480_b200 import workloads  # noqa: E402  (seeded inputs; no method arithmetic)
+
+METRIC = "SHO project+add psi-GB/s(box) at 1 B200 (HBM-roofline metric of BASELINE.json); atom*band projections/s in detail"
+ESZ = {"r64": 8, "c128": 16, "r32": 4, "c64": 8}
+# FP64 pipe peak derived from the guide's unit counts: 148 SMs x 64 FP64 FMA
+# lanes x 2 flop x 1.965 GHz (clocks.max.sm).  DMMA and DFMA share this pipe (measured: 37.1 TFLOP/s both).
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+FP32_PEAK_TFLOPS = 2 * FP64_PEAK_TFLOPS
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0}, "fallback"
+
+
+def geometry(w, boxes=None):
+    """Counts only (no method arithmetic): box points and algorithmic flops of one project (= one add)
+    launch over all atoms and bands.  F = 2 P [ box M + n_z n_x pairs + n_z N_SHO ] per atom and band
+    (first-, second- and third-axis contraction of the separable scheme)."""
+    if boxes is None:
+        import oracle  # only reached from the cpu_baseline / reference legs
+        boxes = np.zeros((w.natoms, 3, 2), np.int64)
+        for a in range(w.natoms):
+            lo, hi, _ = oracle.box(w.ng, w.h, w.periodic, w.pos[a], w.sigma[a], w.rcut_sigma)
+            boxes[a, :, 0], boxes[a, :, 1] = lo, hi
+    n = np.maximum(boxes[:, :, 1].astype(np.int64) - boxes[:, :, 0] + 1, 0)
+    box = n[:, 0] * n[:, 1] * n[:, 2]
+    M = w.numax + 1
+    pairs, nsho = M * (M + 1) // 2, M * (M + 1) * (M + 2) // 6
+    P = 2 if w.is_complex else 1
+    flops_atom = 2.0 * P * (box * M + n[:, 2] * n[:, 0] * pairs * (box > 0) + n[:, 2] * nsho * (box > 0))
+    return {"box_points": box, "sum_box": int(box.sum()), "flops_per_band": float(flops_atom.sum()),
+            "nsho": nsho, "P": P}
+
+
+class ClockSampler:
+    """nvidia-smi sampled DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w_max=float(max(pw)),
+                       samples=len(sm), reasons=sorted(reasons))
+        return out
+
+
+# --------------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline of our arm; the whole of --impl reference)
+
+
+def oracle_sample_setup(w, cpu_seconds=20.0):
+    """A bounded sample of the workload for the oracle: the first n_a atoms x n_b bands, sized for about
+    ``cpu_seconds`` core-seconds (project + add)."""
+    import oracle
+    cores = oracle.num_threads()
+    g = geometry(w)
+    n_b = min(w.nbands, cores)
+    rate = (2.5e8 if w.is_complex else 5.0e8)                 # rough oracle speed, box-point*coefficients / s / core
+    t_pair = 2.0 * float(np.mean(g["box_points"])) * g["nsho"] / rate
+    n_a = int(max(1, min(w.natoms, round(cpu_seconds / max(t_pair * n_b, 1e-9)))))
+    psi = w.psi(range(n_b))
+    if w.psi_dist == "zero":
+        psi = workloads.Workload(**{**w.__dict__, "psi_dist": "normal"}).psi(range(n_b))
+    wide = np.complex128 if w.is_complex else np.float64
+    psi = psi.astype(wide)
+    sub_box = int(g["box_points"][:n_a].sum()) * n_b
+    return {"n_a": n_a, "n_b": n_b, "psi": psi, "cores": cores, "box_band_points": sub_box,
+            "bytes": 3.0 * sub_box * ESZ[w.dtype],
+            "sample": "first %d atoms x %d bands of %s: oracle project (direct triple sum) then oracle add" % (n_a, n_b, w.name)}
+
+
+def oracle_sample_run(w, s):
+    import oracle
+    n_a = s["n_a"]
+    t0 = time.perf_counter()
+    c = oracle.project(w.ng, w.h, w.periodic, w.kfrac, w.pos[:n_a], w.sigma[:n_a], w.numax, s["psi"], w.rcut_sigma)
+    oracle.add(w.ng, w.h, w.periodic, w.kfrac, w.pos[:n_a], w.sigma[:n_a], w.numax, c, s["psi"], w.rcut_sigma)
+    return time.perf_counter() - t0
+
+
+def run_reference(args, w):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    s = oracle_sample_setup(w, cpu_seconds=args.ref_cpu_seconds)
+    for _ in range(args.warmup):
+        oracle_sample_run(w, s)
+    ts = [oracle_sample_run(w, s) for _ in range(args.steps)]
+    t = float(np.sum(ts))
+    value = s["bytes"] * args.steps / t / 1e9
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": {"r64": "f64", "c128": "c128", "r32": "f32", "c64": "c64"}[w.dtype], "data": "synthetic",
+        "config": {"workload": w.name, "note": "CPU oracle on a bounded sample of the workload"},
+        "cpu_baseline": {"value": value, "unit": "GB/s", "cores": s["cores"], "kind": "oracle", "sample": s["sample"]},
+        "e2e": {"value": value, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "atom_band_per_s": s["n_a"] * s["n_b"] * args.steps / t,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# --------------------------------------------------------------------------------------------------
+
+
+def run_ours(args, w):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1905_00480_b200 as sho
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    sho.lib()                                                        # fail loudly if libsho.so is missing
+
+    plan = sho.plan_for(w)
+    info = plan.info()
+    g = geometry(w, plan.boxes())
+    nb, esz, P = w.nbands, ESZ[w.dtype], g["P"]
+    tdt = {"r64": torch.float64, "c128": torch.complex128, "r32": torch.float32, "c64": torch.complex64}[w.dtype]
+    # weak scaling over bands: every rank owns nbands bands of its own, seeded per rank
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(w.seed * 1000 + rank)
+    shape = (nb, w.ng[2], w.ng[1], w.ng[0])
+    psi = torch.randn(shape, dtype=tdt, device=dev, generator=gen)   # read by project
+    psi_out = torch.zeros(shape, dtype=tdt, device=dev)             # accumulated into by add (stays finite)
+    coeff = plan.new_coeff(nb, dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        plan.project(psi, coeff, stream)
+        plan.add(coeff, psi_out, stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    sampler = ClockSampler(local) if rank == 0 else None
+    barrier()
+    for k in range(args.steps):
+        ev[k][0].record(stream)
+        plan.project(psi, coeff, stream)
+        ev[k][1].record(stream)
+        plan.add(coeff, psi_out, stream)
+        ev[k][2].record(stream)
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    t_total = ev[0][0].elapsed_time(ev[-1][2]) * 1e-3
+    t_prj = float(np.mean([e[0].elapsed_time(e[1]) for e in ev])) * 1e-3
+    t_add = float(np.mean([e[1].elapsed_time(e[2]) for e in ev])) * 1e-3
+    if world > 1:
+        tt = torch.tensor([t_total, t_prj, t_add], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_total, t_prj, t_add = (float(x) for x in tt.cpu())
+
+    box_bytes = float(g["sum_box"]) * nb * esz                        # B_box of one rank
+    step_bytes = 3.0 * box_bytes * world
+    value = step_bytes * args.steps / t_total / 1e9
+    peaks, peak_kind = measured_peaks()
+    F = g["flops_per_band"] * nb                                     # algorithmic flops of one project (= one add) launch
+    dom, t_dom = ("sho_add_kernel", t_add) if t_add >= t_prj else ("sho_project_kernel", t_prj)
+    alu_peak = FP64_PEAK_TFLOPS                                      # arithmetic is fp64 for all four dtypes
+    roofline = {"bound": "alu", "kernel": dom, "achieved": F / t_dom / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
+                "frac": F / t_dom / 1e12 / alu_peak, "traffic": None,
+                "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md); DMMA/DFMA micro-benchmark in fp64_peak_measured_tflops",
+                "flops_per_launch": F}
+
+    # ---- end to end through the HOST-buffer C-ABI calls (pinned host memory) ----
+    e2e = None
+    if not args.no_e2e:
+        hp = torch.empty(shape, dtype=tdt, pin_memory=True)
+        hc = torch.empty((w.natoms, nb, plan.nsho), dtype=tdt, pin_memory=True)
+        hp.copy_(psi)
+        torch.cuda.synchronize()
+        ke = max(1, min(args.steps, args.e2e_steps))
+        plan.project_host(hp, hc, stream); plan.add_host(hc, hp, stream)      # warm-up (allocates the plan workspace)
+        hp.copy_(psi)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            plan.project_host(hp, hc, stream)
+            plan.add_host(hc, hp, stream)
+        torch.cuda.synchronize()
+        te = time.perf_counter() - t0
+        if world > 1:
+            tt = torch.tensor([te], dtype=torch.float64, device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            te = float(tt.cpu()[0])
+        psi_b, c_b = int(np.prod(shape)) * esz, w.natoms * nb * plan.nsho * esz
+        e2e = {"value": step_bytes * ke / te / 1e9, "unit": "GB/s", "h2d_bytes_per_step": 2 * psi_b + c_b,
+               "d2h_bytes_per_step": psi_b + c_b, "steps": ke, "ms_per_step": 1e3 * te / ke}
+        del hp, hc
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    fp64_meas = sho.measure_fp64_peak(20000) / 1e12
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        s = oracle_sample_setup(w, cpu_seconds=args.ref_cpu_seconds)
+        tc = oracle_sample_run(w, s)
+        cpu = {"value": s["bytes"] / tc / 1e9, "unit": "GB/s", "cores": s["cores"], "kind": "oracle", "sample": s["sample"],
+               "seconds": tc, "atom_band_per_s": s["n_a"] * s["n_b"] / tc}
+    line = {
+        "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": {"r64": "f64", "c128": "c128", "r32": "f32", "c64": "c64"}[w.dtype], "data": "synthetic",
+        "config": {"workload": w.name, "grid": list(w.ng), "h": w.h, "natoms": w.natoms, "numax": w.numax, "nbands_per_gpu": nb,
+                   "elem": w.dtype, "l2": "inputs larger than L2 (psi %.2f GB per GPU)" % (np.prod(shape) * esz / 1e9)
+                   if np.prod(shape) * esz > 2.5e8 else "psi smaller than L2: L2-resident by design of the config",
+                   "sharding": "bands (weak): each rank runs the config's nbands on its own psi, no collective"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps, "roofline": roofline, "cpu_baseline": cpu,
+        "detail": {
+            "ms_project": 1e3 * t_prj, "ms_add": 1e3 * t_add,
+            "psi_gbs_box_project": box_bytes / t_prj / 1e9, "psi_gbs_box_add": 2 * box_bytes / t_add / 1e9,
+            "frac_hbm_peak_project": box_bytes / t_prj / 1e9 / peaks["hbm_gbs"], "frac_hbm_peak_add": 2 * box_bytes / t_add / 1e9 / peaks["hbm_gbs"],
+            "frac_hbm_peak_step": value / world / peaks["hbm_gbs"], "hbm_peak_gbs": peaks["hbm_gbs"], "hbm_peak_kind": peak_kind,
+            "atom_band_per_s": world * info["atoms_nonempty"] * nb * args.steps / t_total,
+            "tflops_project": F / t_prj / 1e12, "tflops_add": F / t_add / 1e12, "fp64_peak_measured_tflops": fp64_meas,
+            "sum_box_points": g["sum_box"], "psi_bytes_unique": int(np.prod(shape)) * esz, "add_tile_pairs": info["add_pairs"],
+        },
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5 (default: the largest, cfg 5)")
+    ap.add_argument("--dtype", default=None, help="override the config's element type (cfg 4: r32 or r64)")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-cpu-seconds", type=float, default=20.0)
+    args = ap.parse_args()
+    w = workloads.make(args.config, dtype=args.dtype)
+    if args.dtype in ("r32", "r64"):
+        w.kfrac = None
+    if args.impl == "reference":
+        return run_reference(args, w)
+    return run_ours(args, w)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
