@@ -2,27 +2,27 @@
 //
 //   psi_b(r) += sum_a sum_n c[a][b][n] phi_nx(x-X_a) phi_ny(y-Y_a) phi_nz(z-Z_a)        step (3)
 //
-// One CTA owns one psi tile of kAddTX x kAddTY x kAddTZ grid points of one band and keeps it in the
-// accumulator registers of its FP64 tensor-core MMAs for the whole kernel; it walks the plan's list
-// of (atom, periodic image) pairs whose box touches the tile, in ascending atom order, and finally
-// does ONE read-modify-write of the tile.  No atomics, bit-reproducible, psi traffic = read + write
-// of every touched tile exactly once.
+// One CTA owns one psi tile of kAddTX x kAddTY x kAddTZ = 8 x 64 x 16 grid points of one band and keeps
+// it in the accumulator registers of its FP64 tensor-core MMAs for the whole kernel; it walks the plan's
+// list of (atom, periodic image) pairs whose box touches the tile, in ascending atom order, and finally
+// does ONE read-modify-write of the tile.  No atomics, bit-reproducible, psi traffic = read + write of
+// every touched tile exactly once.  Warp w owns z plane w of the tile (64 rows x 8 columns).
 //
-// Per (tile, atom image) the expansion runs z -> x -> y:
-//   tables  (CTA-wide, per batch of kAddBatch pairs) the three 1D Hermite-Gauss tables are sampled on
-//           the fly (eq. (31)) into shared memory, laid out as DMMA fragments
-//   z       T2[z][ny][nx] = conj(w) sum_nz c[n(nx,ny,nz)] phi_nz(z)      (plain FMAs, N_SHO per plane)
-//   x       T1[ny][x]     = sum_nx T2[z][ny][nx] phi_nx(x)               DMMA: M = x, K = nx, N = ny
-//   y       psi[y][x]    += sum_ny phi_ny(y) T1[ny][x]                   DMMA: M = y, K = ny, N = x
+// Per batch of (tile, atom image) pairs:
+//   tables  (CTA-wide) the three 1D Hermite-Gauss tables of every pair are sampled on the fly (eq. (31),
+//           PAPER.md:283-286) into shared memory, x and y laid out as DMMA A fragments; the pair's
+//           coefficients c[a][b][:] are staged next to them with coalesced loads
+// then every warp, for every pair of the batch that touches its plane, expands z -> x -> y:
+//   z       T2[ny][nx] = conj(w) sum_nz c[n(nx,ny,nz)] phi_nz(z)         plain FMAs, each lane computes
+//                                                                       exactly the B-fragment entries it needs
+//   x       T1[x][ny]  = sum_nx phi_nx(x) T2[ny][nx]                     DMMA: M = x, K = nx, N = ny
+//   y       psi[y][x] += sum_ny phi_ny(y) T1[x][ny]                      DMMA: M = y, K = ny, N = x
 // The accumulator fragment of the x stage is exactly the B fragment of the y stage when column 2t+s of
 // the x stage's N tile is assigned ny = 8 nt + 4 s + t: the contracted index is then cut in K steps of
 // four consecutive ny, so only ceil((numax+1)/4) steps are issued.
-// Warp w of the CTA owns z plane w / 4 and the 8 columns (w % 4) * 8 .. +7 of the tile, all 64 rows.
 #include "sho_device.cuh"
 
 namespace sho {
-
-constexpr int kAddBatch = 4;
 
 struct AddParams {
     GridDev g;
@@ -36,6 +36,7 @@ struct AddParams {
     int32_t nbands;
     int32_t ntile0, ntile1;
     int32_t vec_ok;
+    int32_t batch;             // pairs per batch (shared-memory slots)
     long long band_stride;
 };
 
@@ -43,37 +44,31 @@ template <int MT, int DT>
 struct AddSmem {
     static constexpr int P = Elem<DT>::cplx ? 2 : 1;
     static constexpr int MP = 8 * MT, KS = 2 * MT;
-    static constexpr int FY = (kAddTY / 8) * KS * 32;              // doubles per entry
-    static constexpr int FX = (kAddTX / 8) * KS * 32;
-    static constexpr int T2 = kAddTZ * P * MT * KS * 32;
+    static constexpr int FY = (kAddTY / 8) * KS * 32;              // doubles per pair
+    static constexpr int FX = KS * 32;
     static constexpr int FZ = kAddTZ * MP;
-    static constexpr int PH = 2;
-    static constexpr int META = 4;                                 // ints
-    static constexpr size_t bytes = (size_t)kAddBatch * ((FY + FX + T2 + FZ + PH) * 8 + META * 4);
+    static constexpr int HEAD = 4;                                 // conj(w) re, im; 4 ints of overlap ranges
+    static __host__ __device__ int slot_doubles(int nsho) { return FY + FX + FZ + HEAD + ((nsho * P + 1) & ~1); }
 };
 
 template <int MT, int DT>
-__global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddParams p)
+__global__ void __launch_bounds__(kAddWarps * 32, 1) sho_add_kernel(const AddParams p)
 {
     using E = Elem<DT>;
     using real_t = typename E::real_t;
     using S = AddSmem<MT, DT>;
     constexpr bool CPLX = E::cplx;
     constexpr int P = S::P, MP = S::MP, KSMAX = S::KS;
-    constexpr int NB = kAddBatch;
-    constexpr int NYT = kAddTY / 8, NXB = kAddTX / 8;
+    constexpr int NYT = kAddTY / 8;
+    static_assert(kAddTX == 8, "one 8-column block per tile");
 
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    double* fyA = reinterpret_cast<double*>(smem_raw);          // [NB][NYT][KS][32]   A fragments of the y stage
-    double* fxA = fyA + NB * S::FY;                             // [NB][NXB][KS][32]   A fragments of the x stage
-    double* t2B = fxA + NB * S::FX;                             // [NB][TZ][P][MT][KS][32]  B fragments of the x stage
-    double* fzs = t2B + NB * S::T2;                             // [NB][TZ][MP]
-    double* phs = fzs + NB * S::FZ;                             // [NB][2]  conj(w) of the image
-    int32_t* meta = reinterpret_cast<int32_t*>(phs + NB * S::PH);   // [NB][4]  yt_lo, yt_hi, x-block mask, z mask
+    extern __shared__ __align__(16) double smem[];
+    const int nsho = p.g.nsho;
+    const int SLOT = S::slot_doubles(nsho);
+    // slot layout: [FY fyA][FX fxA][FZ fzs][2 phase][4 ints meta][nsho*P coefficients]
 
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31, zl = tid >> 5;
     const int q = lane >> 2, t = lane & 3;
-    const int zl = warp / NXB, xb = warp % NXB;
 
     const int b = blockIdx.x / p.n_tile_list;
     const int tile = p.tile_list[blockIdx.x - b * p.n_tile_list];
@@ -83,6 +78,7 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
     const int numax = p.g.numax;
     const int KQ = (numax + 4) >> 2;                            // K steps of four n values that hold n <= numax
     const int ebeg = p.tile_ptr[tile], eend = p.tile_ptr[tile + 1];
+    const int NB = p.batch;
 
     double D[NYT][P][2];
 #pragma unroll
@@ -91,130 +87,126 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
         for (int pp = 0; pp < P; ++pp) D[yt][pp][0] = D[yt][pp][1] = 0.0;
 
     const real_t* cbase = reinterpret_cast<const real_t*>(p.coeff);
+    // (ny, nx) of the B-fragment entries this lane computes in the z stage: B[k = t][col = q]
+    const int ny_l = 4 * (q & 1) + (q >> 1);                    // + 8 nt
 
     for (int e0 = ebeg; e0 < eend; e0 += NB) {
         const int nb = min(NB, eend - e0);
         __syncthreads();                                        // the previous batch's tables are no longer read
-        // ---------------- tables, phase A: 1D functions (step a1), image phase, overlap ranges ----------------
-        constexpr int ITEMS_A = kAddTY + kAddTX + kAddTZ + 1;
-        for (int it = tid; it < nb * ITEMS_A; it += blockDim.x) {
-            const int i = it / ITEMS_A, r = it - i * ITEMS_A;
+        // ---------------- tables: 1D functions (step a1), image phase, overlap ranges ----------------
+        constexpr int ITEMS = kAddTY + kAddTX + kAddTZ + 1;
+        for (int it = tid; it < nb * ITEMS; it += blockDim.x) {
+            const int i = it / ITEMS, r = it - i * ITEMS;
             const AddEntry en = p.tile_ent[e0 + i];
             const AtomDev at = p.atoms[en.atom];
+            double* slot = smem + (size_t)i * SLOT;
             double v[MP];
             if (r < kAddTY) {
                 const int jy = jy0 + r, iy = jy + en.m[1] * Ny;
                 const bool valid = jy < Ny && iy >= at.lo[1] && iy <= at.hi[1];
-                hermite_gauss<MP>(displacement(iy, p.g.h, at.pos[1]), at.sigma, p.g.hnorm, numax, valid, v);
-                const int yt = r >> 3, qq = r & 7;
+                hermite_gauss<MP>(displacement(iy, p.g.h, at.pos[1]), at, p.g.hnorm, numax, valid, v);
+                double* fyA = slot + ((r >> 3) * KSMAX) * 32 + (r & 7) * 4;
 #pragma unroll
-                for (int n = 0; n < MP; ++n)   // A[y = qq][k = n & 3] of K step n >> 2
-                    fyA[((i * NYT + yt) * KSMAX + (n >> 2)) * 32 + qq * 4 + (n & 3)] = v[n];
+                for (int n = 0; n < MP; ++n)   // A[y = r & 7][k = n & 3] of K step n >> 2
+                    fyA[(n >> 2) * 32 + (n & 3)] = v[n];
             } else if (r < kAddTY + kAddTX) {
                 const int cidx = r - kAddTY;
                 const int jx = jx0 + cidx, ix = jx + en.m[0] * Nx;
                 const bool valid = jx < Nx && ix >= at.lo[0] && ix <= at.hi[0];
-                hermite_gauss<MP>(displacement(ix, p.g.h, at.pos[0]), at.sigma, p.g.hnorm, numax, valid, v);
-                const int xbb = cidx >> 3, qq = cidx & 7;
+                hermite_gauss<MP>(displacement(ix, p.g.h, at.pos[0]), at, p.g.hnorm, numax, valid, v);
+                double* fxA = slot + S::FY + cidx * 4;
 #pragma unroll
-                for (int n = 0; n < MP; ++n)   // A[x = qq][k = n & 3] of K step n >> 2
-                    fxA[((i * NXB + xbb) * KSMAX + (n >> 2)) * 32 + qq * 4 + (n & 3)] = v[n];
+                for (int n = 0; n < MP; ++n)   // A[x = cidx][k = n & 3] of K step n >> 2
+                    fxA[(n >> 2) * 32 + (n & 3)] = v[n];
             } else if (r < kAddTY + kAddTX + kAddTZ) {
                 const int z = r - kAddTY - kAddTX;
                 const int jz = jz0 + z, iz = jz + en.m[2] * Nz;
                 const bool valid = jz < Nz && iz >= at.lo[2] && iz <= at.hi[2];
-                hermite_gauss<MP>(displacement(iz, p.g.h, at.pos[2]), at.sigma, p.g.hnorm, numax, valid, v);
+                hermite_gauss<MP>(displacement(iz, p.g.h, at.pos[2]), at, p.g.hnorm, numax, valid, v);
+                double* fzs = slot + S::FY + S::FX + z * MP;
 #pragma unroll
-                for (int n = 0; n < MP; ++n) fzs[(i * kAddTZ + z) * MP + n] = v[n];
+                for (int n = 0; n < MP; ++n) fzs[n] = v[n];
             } else {
                 // overlap of the box with the tile, in units the warps can skip
-                const int oy = jy0 + en.m[1] * Ny, ox = jx0 + en.m[0] * Nx, oz = jz0 + en.m[2] * Nz;
+                const int oy = jy0 + en.m[1] * Ny, oz = jz0 + en.m[2] * Nz;
                 const int ylast = min(kAddTY, Ny - jy0) - 1;
                 const int ya = max(at.lo[1] - oy, 0), yb = min(at.hi[1] - oy, ylast);
-                int xmask = 0, zmask = 0;
-                for (int k = 0; k < NXB; ++k) {
-                    const int c0 = max(ox + 8 * k, at.lo[0]), c1 = min(min(ox + 8 * k + 7, at.hi[0]), Nx - 1 + en.m[0] * Nx);
-                    if (c1 >= c0) xmask |= 1 << k;
-                }
+                int zmask = 0;
                 for (int k = 0; k < kAddTZ; ++k) {
                     const int iz = oz + k;
                     if (jz0 + k < Nz && iz >= at.lo[2] && iz <= at.hi[2]) zmask |= 1 << k;
                 }
-                meta[4 * i + 0] = ya >> 3;
-                meta[4 * i + 1] = (yb >= ya) ? (yb >> 3) : -1;
-                meta[4 * i + 2] = xmask;
-                meta[4 * i + 3] = zmask;
+                double* head = slot + S::FY + S::FX + S::FZ;
                 double sn = 0.0, cs = 1.0;
                 if (CPLX && p.g.has_phase)   // conj(w), w = exp(2 pi i k.m)  (reading A6)
                     sincospi(-2.0 * (p.g.kfrac[0] * en.m[0] + p.g.kfrac[1] * en.m[1] + p.g.kfrac[2] * en.m[2]), &sn, &cs);
-                phs[2 * i] = cs; phs[2 * i + 1] = sn;
+                head[0] = cs; head[1] = sn;
+                int32_t* meta = reinterpret_cast<int32_t*>(head + 2);
+                meta[0] = ya >> 3;
+                meta[1] = (yb >= ya) ? (yb >> 3) : -1;
+                meta[2] = zmask;
+                meta[3] = en.atom;
             }
         }
-        __syncthreads();
-        // ---------------- tables, phase B: z stage, T2 = conj(w) sum_nz c phi_nz(z), as B fragments ----------------
-        const int items_b = kAddTZ * MT * KQ * 32;
-        for (int it = tid; it < nb * items_b; it += blockDim.x) {
-            const int i = it / items_b;
-            int r = it - i * items_b;
-            const int ln = r & 31; r >>= 5;
-            const int ks = r % KQ; r /= KQ;
-            const int nt = r % MT, z = r / MT;
-            const int qq = ln >> 2, tt = ln & 3;
-            const int ny = 8 * nt + 4 * (qq & 1) + (qq >> 1), nx = 4 * ks + tt;   // B[k = tt][col qq]
-            double sre = 0.0, sim = 0.0;
-            if (ny + nx <= numax && ((meta[4 * i + 3] >> z) & 1)) {
-                const AddEntry en = p.tile_ent[e0 + i];
-                const real_t* c = cbase + ((size_t)en.atom * p.nbands + b) * p.g.nsho * P;
-                const double* fz = fzs + (i * kAddTZ + z) * MP;
-                int zoff = 0;
-                for (int nz = 0; nz <= numax - ny - nx; ++nz) {
-                    const int mrow = numax - nz + 1;                                // rows (ny values) in plane nz
-                    const int n = zoff + ny * mrow - (ny * (ny - 1)) / 2 + nx;      // reading A8
-                    if (!CPLX) sre = fma((double)__ldg(c + n), fz[nz], sre);
-                    else {
-                        sre = fma((double)__ldg(c + 2 * n), fz[nz], sre);
-                        sim = fma((double)__ldg(c + 2 * n + 1), fz[nz], sim);
-                    }
-                    zoff += mrow * (mrow + 1) / 2;
-                }
-            }
-            double* dst = t2B + ((((size_t)(i * kAddTZ + z) * P) * MT + nt) * KSMAX + ks) * 32 + ln;
-            if (!CPLX) dst[0] = sre;
-            else {
-                const double cr = phs[2 * i], ci = phs[2 * i + 1];
-                dst[0] = sre * cr - sim * ci;
-                dst[(size_t)MT * KSMAX * 32] = sre * ci + sim * cr;
-            }
-        }
-        __syncthreads();
-        // ---------------- x and y stages on the tensor cores ----------------
+        // coefficients of the batch, coalesced: c[atom][b][0 .. nsho) -> shared (as doubles)
         for (int i = 0; i < nb; ++i) {
-            const int ytlo = meta[4 * i + 0], ythi = meta[4 * i + 1];
-            if (!((meta[4 * i + 2] >> xb) & 1) || !((meta[4 * i + 3] >> zl) & 1) || ythi < ytlo) continue;
+            const int atom = p.tile_ent[e0 + i].atom;
+            const real_t* c = cbase + ((size_t)atom * p.nbands + b) * nsho * P;
+            double* cs = smem + (size_t)i * SLOT + S::FY + S::FX + S::FZ + S::HEAD;
+            for (int n = tid; n < nsho * P; n += blockDim.x) cs[n] = (double)__ldg(c + n);
+        }
+        __syncthreads();
+        // ---------------- z, x and y stages: every warp on its own plane ----------------
+        for (int i = 0; i < nb; ++i) {
+            const double* slot = smem + (size_t)i * SLOT;
+            const double* head = slot + S::FY + S::FX + S::FZ;
+            const int32_t* meta = reinterpret_cast<const int32_t*>(head + 2);
+            const int ytlo = meta[0], ythi = meta[1];
+            if (!((meta[2] >> zl) & 1) || ythi < ytlo) continue;
+            const double* fz = slot + S::FY + S::FX + zl * MP;
+            const double* cs = head + S::HEAD;
+            const double wr = head[0], wi = head[1];
+
             double D1[MT][P][2];
 #pragma unroll
             for (int nt = 0; nt < MT; ++nt)
 #pragma unroll
                 for (int pp = 0; pp < P; ++pp) D1[nt][pp][0] = D1[nt][pp][1] = 0.0;
 #pragma unroll
-            for (int nt = 0; nt < MT; ++nt)
+            for (int nt = 0; nt < MT; ++nt) {
+                const int ny = 8 * nt + ny_l;
 #pragma unroll
-                for (int ks = 0; ks < KSMAX; ++ks)
-                    if (ks < KQ && 8 * nt + 4 * ks <= numax) {
-                        const double a = fxA[((i * NXB + xb) * KSMAX + ks) * 32 + lane];
+                for (int ks = 0; ks < KSMAX; ++ks) {
+                    if (ks < KQ && 8 * nt + 4 * ks <= numax) {          // warp-uniform: the block holds some ny+nx <= numax
+                        const int nx = 4 * ks + t;
+                        const int lim = numax - ny - nx;                // nz <= lim
+                        const int base = ny * (numax + 1) - (ny * (ny - 1)) / 2 + nx;   // reading A8, minus the nz part
+                        double sre = 0.0, sim = 0.0;
 #pragma unroll
-                        for (int pp = 0; pp < P; ++pp) {
-                            const double bb = t2B[((((size_t)(i * kAddTZ + zl) * P + pp) * MT + nt) * KSMAX + ks) * 32 + lane];
-                            dmma(D1[nt][pp][0], D1[nt][pp][1], a, bb);
+                        for (int nz = 0; nz < MP; ++nz) {
+                            if (nz <= lim) {
+                                const int n = base + p.g.zoff[nz] - ny * nz;
+                                const double f = fz[nz];
+                                if (!CPLX) sre = fma(cs[n], f, sre);
+                                else { sre = fma(cs[2 * n], f, sre); sim = fma(cs[2 * n + 1], f, sim); }
+                            }
+                        }
+                        const double a = slot[S::FY + ks * 32 + lane];
+                        if (!CPLX) dmma(D1[nt][0][0], D1[nt][0][1], a, sre);
+                        else {
+                            dmma(D1[nt][0][0], D1[nt][0][1], a, sre * wr - sim * wi);
+                            dmma(D1[nt][P - 1][0], D1[nt][P - 1][1], a, sre * wi + sim * wr);
                         }
                     }
+                }
+            }
 #pragma unroll
             for (int yt = 0; yt < NYT; ++yt)
                 if (yt >= ytlo && yt <= ythi) {
 #pragma unroll
                     for (int kk = 0; kk < KSMAX; ++kk)
                         if (kk < KQ) {
-                            const double a = fyA[((i * NYT + yt) * KSMAX + kk) * 32 + lane];
+                            const double a = slot[(yt * KSMAX + kk) * 32 + lane];
 #pragma unroll
                             for (int pp = 0; pp < P; ++pp) dmma(D[yt][pp][0], D[yt][pp][1], a, D1[kk >> 1][pp][kk & 1]);
                         }
@@ -226,7 +218,7 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
     const int jz = jz0 + zl;
     if (jz < Nz) {
         real_t* pb = reinterpret_cast<real_t*>(p.psi) + ((size_t)b * p.band_stride + (size_t)jz * Ny * Nx) * P;
-        const int jx = jx0 + xb * 8 + 2 * t;
+        const int jx = jx0 + 2 * t;
 #pragma unroll
         for (int yt = 0; yt < NYT; ++yt) {
             const int jy = jy0 + 8 * yt + q;
@@ -278,12 +270,15 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
     const size_t esz = elem_size(pl->dtype);
     const size_t valign = CPLX ? esz : 2 * esz;
     p.vec_ok = ((reinterpret_cast<uintptr_t>(psi) % valign) == 0) && (CPLX || (pl->g.ng[0] % 2 == 0));
+    const size_t slot_bytes = (size_t)S::slot_doubles(pl->g.nsho) * 8;
+    p.batch = (int)std::max<size_t>(1, std::min<size_t>(11, (200 * 1024) / slot_bytes));
+    const size_t smem = slot_bytes * p.batch;
     auto kern = sho_add_kernel<MT, DT>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::bytes);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(add)");
     const long long nblocks = (long long)pl->n_tile_list * nbands;
     if (nblocks > 0x7fffffffLL) { set_error("sho_add: tiles*nbands too large"); return SHO_ERR_UNSUPPORTED; }
-    kern<<<(unsigned)nblocks, kAddWarps * 32, S::bytes, s>>>(p);
+    kern<<<(unsigned)nblocks, kAddWarps * 32, smem, s>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "launch sho_add_kernel");
     return SHO_OK;

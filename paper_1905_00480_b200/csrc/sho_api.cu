@@ -146,6 +146,12 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
         }
     }
 
+    for (int nz = 0, run = 0; nz <= SHO_NUMAX_MAX; ++nz) {
+        g.zoff[nz] = run;
+        const int m = numax - nz + 1;
+        if (m > 0) run += m * (m + 1) / 2;
+    }
+
     // ---- integer box ranges (reading A3/A5), evaluated in IEEE double exactly as written ----
     p->atoms.resize(natoms);
     p->max_n[0] = p->max_n[1] = p->max_n[2] = 0;
@@ -155,6 +161,8 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
         AtomDev& at = p->atoms[a];
         std::memset(&at, 0, sizeof(at));
         at.sigma = sigma[a];
+        at.inv_sigma = 1.0 / sigma[a];
+        at.pref = 1.0 / std::sqrt(1.7724538509055160273 * sigma[a]);     // (sqrt(pi) sigma)^(-1/2)
         bool is_empty = false;
         int64_t npts = 1;
         for (int d = 0; d < 3; ++d) {

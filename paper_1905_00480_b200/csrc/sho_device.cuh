@@ -30,11 +30,11 @@ __device__ __forceinline__ int floordiv(int i, int n)
 // (PAPER.md:286): phi_n = sqrt(2^n/n!) (sqrt(pi) sigma)^(-1/2) H_n(xi) exp(-xi^2/2), xi = u/sigma.
 // Entries with n > numax (or valid == false) are written as exact zeros.
 template <int NMAX>
-__device__ __forceinline__ void hermite_gauss(double u, double sigma, const double* __restrict__ hnorm, int numax,
+__device__ __forceinline__ void hermite_gauss(double u, const AtomDev& at, const double* __restrict__ hnorm, int numax,
                                               bool valid, double (&out)[NMAX])
 {
-    const double xi = u / sigma;
-    const double g = valid ? exp(-0.5 * xi * xi) * rsqrt(1.7724538509055160273 * sigma) : 0.0;
+    const double xi = u * at.inv_sigma;
+    const double g = valid ? exp(-0.5 * xi * xi) * at.pref : 0.0;
     double hm = 0.0, hc = 1.0;
 #pragma unroll
     for (int n = 0; n < NMAX; ++n) {

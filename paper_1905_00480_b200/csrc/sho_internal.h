@@ -11,13 +11,15 @@
 namespace sho {
 
 constexpr int kProjWarps = 8;          // warps per CTA in the project kernel (one z-plane each per round)
-constexpr int kAddTX = 32, kAddTY = 64, kAddTZ = 2;   // psi tile owned by one CTA of the add kernel
-constexpr int kAddWarps = (kAddTX / 8) * kAddTZ;      // one (z, x-block) per warp
+constexpr int kAddTX = 8, kAddTY = 64, kAddTZ = 16;   // psi tile owned by one CTA of the add kernel
+constexpr int kAddWarps = kAddTZ;                     // one z plane (64 rows x 8 columns) per warp
 
-// one atom as the kernels see it (64 bytes)
+// one atom as the kernels see it (80 bytes)
 struct AtomDev {
     double pos[3];
     double sigma;
+    double inv_sigma;   // 1 / sigma
+    double pref;        // (sqrt(pi) sigma)^(-1/2): normalisation of phi_0 (reading A1)
     int32_t lo[3];   // unwrapped inclusive box range per axis (reading A3); lo > hi on any axis: empty
     int32_t hi[3];
     int32_t pad[2];
@@ -35,6 +37,7 @@ struct GridDev {
     double h;
     double kfrac[3];
     double hnorm[SHO_NUMAX_MAX + 1];   // sqrt(2^n / n!): scale of the monic recurrence of eq. (31)
+    int32_t zoff[SHO_NUMAX_MAX + 1];   // coefficients before plane nz of the (nx,ny,nz) enumeration (reading A8)
     int32_t numax;
     int32_t nsho;
     int32_t natoms;

@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
             int iy = (pr < K0 * 4) ? at.lo[1] + pr : yB + (pr - K0 * 4);
             const bool valid = (pr < K0 * 4) ? (iy < yB && iy <= at.hi[1]) : (iy <= at.hi[1]);
             if (!valid) iy = at.hi[1];
-            hermite_gauss<MP>(displacement(iy, p.g.h, at.pos[1]), at.sigma, p.g.hnorm, numax, valid, v);
+            hermite_gauss<MP>(displacement(iy, p.g.h, at.pos[1]), at, p.g.hnorm, numax, valid, v);
             const int k = pr >> 2, tt = pr & 3;
 #pragma unroll
             for (int n = 0; n < MP; ++n) fy[((size_t)k * MT + (n >> 3)) * 32 + (n & 7) * 4 + tt] = v[n];
@@ -119,7 +119,7 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
             const int j = it - ny_items;
             const int ix = xs0 + j;
             const bool valid = ix >= at.lo[0] && ix <= at.hi[0];
-            hermite_gauss<MP>(displacement(ix, p.g.h, at.pos[0]), at.sigma, p.g.hnorm, numax, valid, v);
+            hermite_gauss<MP>(displacement(ix, p.g.h, at.pos[0]), at, p.g.hnorm, numax, valid, v);
             const int c = j / CW, r = j % CW;
             int slot, tt;
             if (!CPLX) { tt = r >> 2; slot = (c * 2 + (r & 1)) * 2 + ((r >> 1) & 1); }   // r = 4t + 2s + e
@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
         } else {
             const int zi = it - ny_items - nx_items;
             const int iz = at.lo[2] + zi;
-            hermite_gauss<MP>(displacement(iz, p.g.h, at.pos[2]), at.sigma, p.g.hnorm, numax, true, v);
+            hermite_gauss<MP>(displacement(iz, p.g.h, at.pos[2]), at, p.g.hnorm, numax, true, v);
 #pragma unroll
             for (int n = 0; n < MP; ++n) fz[(size_t)zi * MP + n] = v[n];
             if (CPLX) {

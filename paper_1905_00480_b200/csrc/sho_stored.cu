@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(256) sho_tables_kernel(GridDev g, const AtomDe
         double v[SHO_NUMAX_MAX + 1];
         const int d = it < nxl ? 0 : it < nxl + nyl ? 1 : 2;
         const int i = d == 0 ? at.lo[0] + it : d == 1 ? at.lo[1] + it - nxl : at.lo[2] + qz;
-        hermite_gauss<SHO_NUMAX_MAX + 1>(displacement(i, g.h, at.pos[d]), at.sigma, g.hnorm, g.numax, true, v);
+        hermite_gauss<SHO_NUMAX_MAX + 1>(displacement(i, g.h, at.pos[d]), at, g.hnorm, g.numax, true, v);
         double* dst = d == 0 ? fx + (size_t)it * M : d == 1 ? fy + (size_t)(it - nxl) * M : fz;
         for (int n = 0; n < M; ++n) dst[n] = v[n];
     }
