@@ -52,9 +52,9 @@ static sho_status upload(T** dst, const std::vector<T>& src, const char* what)
 static void plan_free_device(sho_plan* p)
 {
     cudaFree(p->d_atoms); cudaFree(p->d_order); cudaFree(p->d_nxyz);
-    cudaFree(p->d_tile_ptr); cudaFree(p->d_tile_ent); cudaFree(p->d_tile_list);
+    cudaFree(p->d_tile_ptr); cudaFree(p->d_tile_ent); cudaFree(p->d_tile_list); cudaFree(p->d_cainv);
     cudaFree(p->ws_psi); cudaFree(p->ws_c);
-    p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr;
+    p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr; p->d_cainv = nullptr;
     p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr;
     p->ws_psi = nullptr; p->ws_c = nullptr;
 }
@@ -122,7 +122,7 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
     sho_plan* p = new (std::nothrow) sho_plan();
     if (!p) { set_error("sho_plan_create: host allocation failed"); return SHO_ERR_OOM; }
     p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr;
-    p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr;
+    p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr; p->d_cainv = nullptr;
     p->ws_psi = nullptr; p->ws_c = nullptr; p->ws_psi_bytes = 0; p->ws_c_bytes = 0;
     p->rcut_sigma = rcut_sigma;
     p->dtype = dtype;
@@ -181,6 +181,11 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
             else if (hi - lo + 1 > ng[d]) {
                 set_error("sho_plan_create: atom %d: box of %d points is wider than the periodic cell (%d) on axis %d",
                           a, hi - lo + 1, ng[d], d);
+                delete p;
+                return SHO_ERR_UNSUPPORTED;
+            }
+            if (g.periodic[d] && (std::abs(floordiv_h(lo, ng[d])) > 32000 || std::abs(floordiv_h(hi, ng[d])) > 32000)) {
+                set_error("sho_plan_create: atom %d is more than 32000 cells away from the home cell on axis %d", a, d);
                 delete p;
                 return SHO_ERR_UNSUPPORTED;
             }
@@ -261,7 +266,25 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
                             const int64_t t = ((int64_t)z.tile * p->ntile[1] + y.tile) * p->ntile[0] + x.tile;
                             if (pass == 0) tile_ptr[t + 1] += 1;
                             else {
-                                AddEntry e; e.atom = a; e.m[0] = x.m; e.m[1] = y.m; e.m[2] = z.m;
+                                AddEntry e;
+                                std::memset(&e, 0, sizeof(e));
+                                e.atom = a; e.m[0] = (int16_t)x.m; e.m[1] = (int16_t)y.m; e.m[2] = (int16_t)z.m;
+                                // overlap of the box with the tile, in the units the warps can skip
+                                const int oy = y.tile * kAddTY + y.m * g.ng[1], oz = z.tile * kAddTZ + z.m * g.ng[2];
+                                const int ylast = std::min(kAddTY, g.ng[1] - y.tile * kAddTY) - 1;
+                                const int ya = std::max(at.lo[1] - oy, 0), yb = std::min(at.hi[1] - oy, ylast);
+                                e.ytlo = (int8_t)(ya >> 3); e.ythi = (int8_t)(yb >> 3);
+                                unsigned zm = 0;
+                                for (int k = 0; k < kAddTZ; ++k) {
+                                    const int iz = oz + k;
+                                    if (z.tile * kAddTZ + k < g.ng[2] && iz >= at.lo[2] && iz <= at.hi[2]) zm |= 1u << k;
+                                }
+                                e.zmask = (uint8_t)zm;
+                                // conj(w), w = exp(2 pi i kfrac.m)  (reading A6)
+                                const double ang = -2.0 * 3.14159265358979323846 *
+                                                   (g.kfrac[0] * x.m + g.kfrac[1] * y.m + g.kfrac[2] * z.m);
+                                e.wr = g.has_phase ? std::cos(ang) : 1.0;
+                                e.wi = g.has_phase ? std::sin(ang) : 0.0;
                                 tile_ent[(size_t)fill[t]++] = e;
                             }
                         }
@@ -277,6 +300,31 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
         if (tile_ptr[t + 1] > tile_ptr[t]) tile_list.push_back((int32_t)t);
     p->n_tile_list = (int32_t)tile_list.size();
 
+    // ---- z stage of the add as an MMA: (ny,nx) pairs sorted by s = ny+nx, row tiles of 8 ----
+    std::vector<uint16_t> cainv((size_t)g.nsho, 0);
+    {
+        AddZTiles& zt = p->ztiles;
+        std::memset(&zt, 0, sizeof(zt));
+        const int npair = (numax + 1) * (numax + 2) / 2;
+        zt.nmt = (npair + 7) / 8;
+        int blk = 0;
+        for (int mt = 0; mt < zt.nmt; ++mt) {
+            int s = 0;                                         // s of the first pair of the tile = smallest s
+            while ((s + 1) * (s + 2) / 2 <= 8 * mt) ++s;
+            zt.blk0[mt] = (int8_t)blk;
+            zt.nks[mt] = (int8_t)((numax - s) / 4 + 1);
+            blk += zt.nks[mt];
+        }
+        zt.nblk = blk;
+        for (int nz = 0, n = 0; nz <= numax; ++nz)
+            for (int ny = 0; ny <= numax - nz; ++ny)
+                for (int nx = 0; nx <= numax - nz - ny; ++nx, ++n) {
+                    const int s = ny + nx, pi = s * (s + 1) / 2 + nx;
+                    const int b = zt.blk0[pi >> 3] + (nz >> 2);
+                    cainv[(size_t)n] = (uint16_t)(b * 32 + 4 * (pi & 7) + (nz & 3));
+                }
+    }
+
     // ---- device mirrors ----
     cudaError_t e = cudaGetDevice(&p->device);
     if (e != cudaSuccess) { sho_status s = cuda_fail(e, "sho_plan_create: cudaGetDevice (no CUDA device?)"); delete p; return s; }
@@ -286,7 +334,8 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
         (st = upload(&p->d_nxyz, nxyz, "sho_plan_create: nxyz")) != SHO_OK ||
         (st = upload(&p->d_tile_ptr, tile_ptr, "sho_plan_create: tile_ptr")) != SHO_OK ||
         (st = upload(&p->d_tile_ent, tile_ent, "sho_plan_create: tile_ent")) != SHO_OK ||
-        (st = upload(&p->d_tile_list, tile_list, "sho_plan_create: tile_list")) != SHO_OK) {
+        (st = upload(&p->d_tile_list, tile_list, "sho_plan_create: tile_list")) != SHO_OK ||
+        (st = upload(&p->d_cainv, cainv, "sho_plan_create: cainv")) != SHO_OK) {
         plan_free_device(p);
         delete p;
         return st;

@@ -11,8 +11,9 @@
 namespace sho {
 
 constexpr int kProjWarps = 8;          // warps per CTA in the project kernel (one z-plane each per round)
-constexpr int kAddTX = 8, kAddTY = 64, kAddTZ = 16;   // psi tile owned by one CTA of the add kernel
+constexpr int kAddTX = 8, kAddTY = 64, kAddTZ = 8;    // psi tile owned by one CTA of the add kernel
 constexpr int kAddWarps = kAddTZ;                     // one z plane (64 rows x 8 columns) per warp
+constexpr int kAddMaxMT = 17;                         // (ny,nx) pairs of numax = 15: 136 = 17 MMA row tiles
 
 // one atom as the kernels see it (80 bytes)
 struct AtomDev {
@@ -25,10 +26,23 @@ struct AtomDev {
     int32_t pad[2];
 };
 
-// one (atom image) that overlaps an add tile: unwrapped index i = j + m*N on each axis
+// one (atom image) that overlaps an add tile: unwrapped index i = j + m*N on each axis (32 bytes)
 struct AddEntry {
     int32_t atom;
-    int32_t m[3];
+    int16_t m[3];
+    uint8_t zmask;       // planes of the tile inside the box (bit k = plane k)
+    int8_t ytlo, ythi;   // first / last 8-row block of the tile that the box touches
+    int8_t pad[3];
+    double wr, wi;       // conj(exp(2 pi i kfrac.m)): Bloch phase of the image, conjugated (reading A6)
+};
+
+// the (ny,nx) pairs with ny+nx <= numax, sorted by s = ny+nx (pair index s(s+1)/2 + nx), cut in MMA row
+// tiles of 8: tile mt needs nz <= numax - s_min(mt), i.e. nks[mt] K steps of 4, stored from block blk0[mt]
+struct AddZTiles {
+    int32_t nmt;         // row tiles
+    int32_t nblk;        // sum of nks
+    int8_t blk0[kAddMaxMT];
+    int8_t nks[kAddMaxMT];
 };
 
 struct GridDev {
@@ -68,6 +82,8 @@ struct sho_plan {
     sho::AddEntry* d_tile_ent;             // [npairs]
     int32_t* d_tile_list;                  // tiles with at least one entry
     int32_t n_tile_list;
+    sho::AddZTiles ztiles;
+    uint16_t* d_cainv;                     // [nsho] coefficient n -> slot (block*32 + 4 q + t) of the z-stage A fragments
     // workspace for the *_host calls
     void* ws_psi; size_t ws_psi_bytes;
     void* ws_c;   size_t ws_c_bytes;
