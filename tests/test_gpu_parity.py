@@ -187,6 +187,20 @@ def test_every_numax_tile_shape(sho, numax):
     run_case(sho, _custom(ng, (1, 1, 1), pos, [0.3, 0.36], numax, 2, h=0.3, rc=4.0), stored=numax <= 9)
 
 
+@pytest.mark.parametrize("numax", [8, 9])
+@pytest.mark.parametrize("dtype", ["r64", "r32", "c128", "c64"])
+def test_remainder_rows_every_dtype(sho, numax, dtype):
+    # numax 8, 9: the project kernel runs rows ny, nx = 8, 9 as DFMA partials beside the MMA tile.  Boxes of
+    # ~29 points wrap on x and y (atom near the origin), span several x chunks and a ragged last y group;
+    # complex data carry a Bloch phase on every axis.
+    rng = np.random.default_rng(300 + numax)
+    ng = (44, 40, 36)
+    pos = np.array([[0.4, 0.7, 5.0], [6.1, 5.3, 0.2], [10.2, 9.4, 8.1]])
+    kfrac = (0.1, 0.2, 0.3) if dtype in ("c128", "c64") else None
+    w = _custom(ng, (1, 1, 1), pos, rng.uniform(0.55, 0.62, 3), numax, 2, dtype=dtype, h=0.25, kfrac=kfrac)
+    run_case(sho, w, stored=False)
+
+
 def test_box_exactly_as_wide_as_the_cell(sho):
     # periodic box of exactly N points on x (every grid point once, one wrap)
     ng = (24, 40, 40)
