@@ -3,33 +3,36 @@
 //   c[a][b][n(nx,ny,nz)] = h^3 sum_r psi_b(r) phi_nx(x-X_a) phi_ny(y-Y_a) phi_nz(z-Z_a)
 //                                                       eq. (25)-(26); step (1)
 //
-// Design (B200, sm_100a): the separable contraction runs y -> x -> z.
+// Design (B200, sm_100a): the separable contraction runs x -> y -> z, as the paper's eq. (26) is written.
 //   a1  every CTA samples the three 1D Hermite-Gauss tables of its atom on the fly (eq. (31)) straight
 //       into shared memory, already laid out as FP64 tensor-core fragments; nothing but 80 B of atom
 //       parameters is read from HBM for the projectors.
-//   a2  psi is read straight from global memory / L2 with 16-byte loads: a warp load covers 4 rows x
-//       128 contiguous bytes, and the loaded registers ARE the B fragments of the first contraction
-//       (K = y, N = x contiguous), so no shared-memory staging or transposition is needed.  Periodic
-//       wrap / isolated clipping are per-lane index arithmetic.  The loads run one group of G y steps
-//       ahead of the arithmetic (register double buffer) and the ring runs on across chunk ends and
-//       plane ends, so loads stay in flight over the x stage, a5 and its barrier.
-//   a3  first-axis (y) contraction: DMMA.8x8x4, M = ny, K = 4 rows, N = 8 columns.  With numax = 8, 9
+//   a2  psi is read straight from global memory / L2 with 32-byte loads (LDG.256): lane (q,t) of a warp
+//       reads 32 contiguous bytes of row q, four lanes cover one 128-byte line, a warp load covers
+//       8 rows x 128 B.  The loaded registers ARE the B fragments of the first contraction (K = x,
+//       N = 8 rows), so no shared-memory staging or transposition is needed, and the L1 data pipe moves
+//       a full line per wavefront (the earlier K = y layout touched 16 lines per 512 B and was bound by
+//       that pipe: profiles/r1_v2_cfg5_project_ncu_full.txt).  Periodic wrap / isolated clipping are
+//       per-lane index arithmetic from two small offset tables.  The loads run one group of G steps
+//       ahead of the arithmetic (register double buffer) and the ring runs on across row-block ends and
+//       plane ends, so loads stay in flight over the y stage, a5 and its barrier.
+//   a3  first-axis (x) contraction: DMMA.8x8x4, M = nx, K = 4 columns, N = 8 rows.  With numax = 8, 9
 //       (M = 9, 10) a second, mostly empty MMA row tile would cost 1.6x the algorithmic flops, so the
-//       R = 2 remainder rows ny = 8, 9 run as plain DFMAs on the same loaded values instead (template
-//       parameter R): per lane a partial over its own row, reduced once per plane.
-//   a4  second-axis (x) contraction: the accumulator fragment of a3 is directly the A fragment of a
-//       second DMMA against the phi_nx table (the K order inside an MMA is free).  For R = 2 the six
-//       (ny,nx) outputs with ny or nx in {8, 9} are DFMA partials per lane.
-//   a5  third axis: each warp owns one z-plane per round; the per-plane T2[ny][nx] meet in shared
-//       memory and thread n accumulates c[n] += phi_nz(z) * T2[ny][nx] in a register.  One
+//       R = 2 remainder rows nx = 8, 9 run as plain DFMAs on the same loaded values instead (template
+//       parameter R): per lane a partial over its own columns, reduced once per plane.
+//   a4  second-axis (y) contraction: the accumulator fragment of a3 is directly the A fragment of a
+//       second DMMA against the phi_ny table (the K order inside an MMA is free).  For R = 2 the six
+//       (nx,ny) outputs with nx or ny in {8, 9} are DFMA partials per lane.
+//   a5  third axis: each warp owns one z-plane per round; the per-plane T2[nx][ny] meet in shared
+//       memory and thread n accumulates c[n] += phi_nz(z) * T2[nx][ny] in a register.  One
 //       __syncthreads per round (double-buffered), coalesced store of N_SHO coefficients at the end.
-// Bloch phases never touch the inner loop: x-phases rotate the a3 accumulators per column, the y-phase
-// is a single accumulator rotation at the wrap row, the z-phase is folded into a5.
+// Bloch phases never touch the inner loop: the x-phase is one accumulator rotation at the wrap column,
+// y-phases rotate the a3 accumulators per row, the z-phase (and the last x image) is folded into a5.
 #include "sho_device.cuh"
 
 namespace sho {
 
-constexpr int kProjG = 4;      // y steps (of 4 rows x 8/16 columns) per group of the register load ring
+constexpr int kProjG = 2;      // loads (of 8 rows x 128 B) per group of the register load ring
 
 struct ProjParams {
     GridDev g;
@@ -40,41 +43,64 @@ struct ProjParams {
     const uint32_t* nxyz;
     int32_t nbands;
     int32_t n_work_atoms;      // atoms with a non-empty box (first entries of order[])
-    int32_t ky_cap, nxe_cap, nz_cap;   // capacities of the shared tables (from the plan's largest box)
-    int32_t vec_ok;            // 16-byte (8-byte for fp32) loads are aligned
+    int32_t kx_cap, yb_cap, nz_cap;    // capacities of the shared tables: x steps, 8-row blocks, planes
+    int32_t fast;              // 32-byte loads are legal: psi 32-byte aligned and Nx a multiple of the lane span
     long long band_stride;     // elements between bands
 };
+
+// per element type: EPL elements of 32 bytes per lane and load; a step covers CWX = 4 EPL columns
+template <int DT> struct ProjElem;
+template <> struct ProjElem<SHO_C128> { static constexpr int EPL = 2; };
+template <> struct ProjElem<SHO_R64>  { static constexpr int EPL = 4; };
+template <> struct ProjElem<SHO_C64>  { static constexpr int EPL = 4; };
+template <> struct ProjElem<SHO_R32>  { static constexpr int EPL = 8; };
 
 // shared-memory carve-up (doubles unless noted); every block starts 16-byte aligned
 template <int MT, int R, int DT>
 struct ProjSmem {
     static constexpr int P = Elem<DT>::cplx ? 2 : 1;
-    static constexpr int MP = 8 * MT;                       // ny / nx rows on the MMA
+    static constexpr int EPL = ProjElem<DT>::EPL;
+    static constexpr int CWX = 4 * EPL;
+    static constexpr int MP = 8 * MT;                       // nx / ny rows on the MMA
     static constexpr int NV = MP + R;                       // functions sampled per point
     static constexpr int TS = MP * MP + (R ? 8 : 0);        // one part of one plane's T2 (+ the R specials)
-    static __host__ __device__ size_t fy(int ky) { return (size_t)ky * MT * 32; }
-    static __host__ __device__ size_t fyr(int ky) { return R ? (size_t)ky * 4 * 2 : 0; }
-    static __host__ __device__ size_t fx(int nxe) { return (size_t)nxe * MT * 32; }
-    static __host__ __device__ size_t fxs(int nxe) { return R ? (size_t)nxe * 4 * 4 : 0; }
+    static __host__ __device__ size_t fx(int kx) { return (size_t)kx * EPL * MT * 32; }       // A fragments, x stage
+    static __host__ __device__ size_t fxr(int kx) { return R ? (size_t)kx * CWX * 2 : 0; }    // phi_8, phi_9 per column
+    static __host__ __device__ size_t fy(int yb) { return (size_t)yb * 2 * MT * 32; }         // B fragments, y stage
+    static __host__ __device__ size_t fys(int yb) { return R ? (size_t)yb * 8 * 4 : 0; }      // phi_0,1,8,9 per row
+    static __host__ __device__ size_t wy(int yb) { return Elem<DT>::cplx ? (size_t)yb * 8 * 2 : 0; }
     static __host__ __device__ size_t fz(int nz) { return (size_t)nz * NV + (((size_t)nz * NV) & 1); }
     static __host__ __device__ size_t wz(int nz) { return Elem<DT>::cplx ? (size_t)nz * 2 : 0; }
     static __host__ __device__ size_t t2() { return (size_t)2 * kProjWarps * P * TS; }
-    static __host__ __device__ size_t total_bytes(int ky, int nxe, int nz)
+    static __host__ __device__ size_t ints(int kx, int yb) { return (size_t)yb * 8 + (size_t)(kx + kProjG) * 4 + 4; }
+    static __host__ __device__ size_t total_bytes(int kx, int yb, int nz)
     {
-        return 8 * (fy(ky) + fyr(ky) + fx(nxe) + fxs(nxe) + fz(nz) + wz(nz) + t2() + 6) + (size_t)(ky + 4) * 4 * 4 + 16;
+        return 8 * (fx(kx) + fxr(kx) + fy(yb) + fys(yb) + wy(yb) + fz(nz) + wz(nz) + t2() + 2) + 4 * ints(kx, yb) + 16;
     }
 };
 
-// position of T2[ny][nx] inside one part of a plane's shared T2 block
+// position of T2[nx][ny] inside one part of a plane's shared T2 block
 template <int MT, int R>
-__device__ __forceinline__ int t2_index(int ny, int nx)
+__device__ __forceinline__ int t2_index(int nx, int ny)
 {
     constexpr int MP = 8 * MT;
-    if (R == 0 || (ny < MP && nx < MP)) return ny * MP + nx;
-    if (ny == MP) return MP * MP + nx;            // (8,0) (8,1)
-    if (ny == MP + 1) return MP * MP + 2;         // (9,0)
-    if (nx == MP) return MP * MP + 3 + 2 * ny;    // (0,8) -> 3, (1,8) -> 5
+    if (R == 0 || (nx < MP && ny < MP)) return nx * MP + ny;
+    if (nx == MP) return MP * MP + ny;            // (8,0) (8,1)
+    if (nx == MP + 1) return MP * MP + 2;         // (9,0)
+    if (ny == MP) return MP * MP + 3 + 2 * nx;    // (0,8) -> 3, (1,8) -> 5
     return MP * MP + 4;                           // (0,9)
+}
+
+// 32 bytes per lane, read-only path (SASS: LDG.E.256.CONSTANT)
+__device__ __forceinline__ void ldg256(const double* p, double (&r)[4])
+{
+    asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(r[0]), "=d"(r[1]), "=d"(r[2]), "=d"(r[3]) : "l"(p));
+}
+__device__ __forceinline__ void ldg256(const float* p, float (&r)[8])
+{
+    asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3]), "=f"(r[4]), "=f"(r[5]), "=f"(r[6]), "=f"(r[7])
+                 : "l"(p));
 }
 
 template <int MT, int R, int DT, int G>
@@ -85,21 +111,23 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
     using real_t = typename E::real_t;
     constexpr bool CPLX = E::cplx;
     constexpr int P = CPLX ? 2 : 1;
+    constexpr int EPL = S::EPL, CWX = S::CWX;
+    constexpr int RAW = 32 / (int)sizeof(real_t);           // reals per lane and load
     constexpr int MP = S::MP, NV = S::NV, TS = S::TS;
-    constexpr int CW = E::cw;                 // columns per chunk (one 16-byte load per lane = 2 MMAs)
-    constexpr int XALIGN = CPLX ? 2 : 4;
     constexpr int NACC = (MT == 1) ? 1 : (816 + kProjWarps * 32 - 1) / (kProjWarps * 32);   // numax <= 9: N_SHO <= 220
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double* fy = reinterpret_cast<double*>(smem_raw);                 // [k][mt][32]   A fragments of the y stage
-    double* fyr = fy + S::fy(p.ky_cap);                               // [row][2]      phi_8, phi_9 of the R rows
-    double* fx = fyr + S::fyr(p.ky_cap);                              // [slot][mt][32] B fragments of the x stage
-    double* fxs = fx + S::fx(p.nxe_cap);                              // [column][4]   phi_0, phi_1, phi_8, phi_9
-    double* fz = fxs + S::fxs(p.nxe_cap);                             // [z][NV]
+    double* fx = reinterpret_cast<double*>(smem_raw);                 // [step][e][mt][32]  A fragments of the x stage
+    double* fxr = fx + S::fx(p.kx_cap);                               // [column][2]        phi_8, phi_9 of the R rows
+    double* fy = fxr + S::fxr(p.kx_cap);                              // [block][s][mt][32] B fragments of the y stage
+    double* fys = fy + S::fy(p.yb_cap);                               // [row][4]           phi_0, phi_1, phi_8, phi_9
+    double* wy = fys + S::fys(p.yb_cap);                              // complex only: [row][2] Bloch phase of the row
+    double* fz = wy + S::wy(p.yb_cap);                                // [z][NV]
     double* wz = fz + S::fz(p.nz_cap);                                // complex only: [z][2]
     double* t2s = wz + S::wz(p.nz_cap);                               // [2][W][P][TS]
-    double* phx = t2s + S::t2();                                      // [2 images][re,im] + y rotation [re,im]
-    int32_t* rowoff = reinterpret_cast<int32_t*>(phx + 6);            // [padded row] element offset of the row
+    double* phx = t2s + S::t2();                                      // x rotation exp(-2 pi i kfrac_x) [re,im]
+    int32_t* rowoff = reinterpret_cast<int32_t*>(phx + 2);            // [padded row] element offset of the row
+    int32_t* coloff = rowoff + (size_t)p.yb_cap * 8;                  // [group][t][step in group] element offset of the lane span
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int q = lane >> 2, t = lane & 3;
@@ -110,68 +138,68 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
     const AtomDev at = p.atoms[a];
     const int Nx = p.g.ng[0], Ny = p.g.ng[1], Nz = p.g.ng[2];
     const int numax = p.g.numax;
+    const bool fast = p.fast != 0;
 
-    const int nzl = at.hi[2] - at.lo[2] + 1;
-    // x: chunks of CW columns starting at a sector-aligned column
-    const int xs0 = floordiv(at.lo[0], XALIGN) * XALIGN;
-    const int XC = (at.hi[0] - xs0 + CW) / CW;
-    // y: K steps of 4 rows; complex data with a y-wrap split the rows at the wrap (one accumulator rotation)
-    int yB = at.hi[1] + 1;   // first row of the second segment (unwrapped); hi+1 = no split
-    if (CPLX && p.g.has_phase && p.g.periodic[1] && p.g.kfrac[1] != 0.0) {
-        const int mlo = floordiv(at.lo[1], Ny), mhi = floordiv(at.hi[1], Ny);
-        if (mhi != mlo) yB = mhi * Ny;
+    const int nyl = at.hi[1] - at.lo[1] + 1, nzl = at.hi[2] - at.lo[2] + 1;
+    // x: steps of CWX columns (one 128-byte line per row) starting at a line-aligned column
+    const int xs0 = floordiv(at.lo[0], CWX) * CWX;
+    const int KX = (at.hi[0] - xs0 + CWX) / CWX;
+    const int KXG = (KX + G - 1) / G;
+    // y: blocks of 8 rows (the N extent of the x-stage MMA)
+    const int NYB = (nyl + 7) >> 3;
+    // complex data with an x-wrap: the accumulators are rotated once, at the first step that holds a column
+    // of the second image; the phase of the last image is folded into wz
+    const bool xphase = CPLX && p.g.has_phase && p.g.periodic[0] && p.g.kfrac[0] != 0.0;
+    const bool yphase = CPLX && p.g.has_phase && p.g.periodic[1] && p.g.kfrac[1] != 0.0;
+    int xB = INT_MAX, kx_rot = -1;
+    if (xphase) {
+        const int mlo = floordiv(at.lo[0], Nx);
+        if (floordiv(at.hi[0], Nx) != mlo) { xB = (mlo + 1) * Nx; kx_rot = (xB - xs0) / CWX; }
     }
-    const int K0 = (min(yB, at.hi[1] + 1) - at.lo[1] + 3) >> 2;
-    const int K1 = (at.hi[1] + 1 - yB + 3) >> 2;          // 0 when there is no split
-    const int KY = K0 + (K1 > 0 ? K1 : 0);
-    const int krot = (K1 > 0) ? K0 : -1;
 
     // ---------------- a1: sample the 1D tables on the fly, in fragment layout ----------------
-    const int KG = (KY + G - 1) / G;            // groups of G y steps (the load ring's granularity)
-    const int ny_items = KG * G * 4, nx_items = XC * CW;
-    for (int it = tid; it < ny_items + nx_items + nzl; it += blockDim.x) {
+    const int nx_items = KX * CWX, ny_items = NYB * 8;
+    for (int it = tid; it < nx_items + ny_items + nzl; it += blockDim.x) {
         double v[NV];
-        if (it < ny_items) {
-            const int pr = it;                                   // padded row slot
-            int iy = (pr < K0 * 4) ? at.lo[1] + pr : yB + (pr - K0 * 4);
-            const bool valid = (pr < K0 * 4) ? (iy < yB && iy <= at.hi[1]) : (iy <= at.hi[1]);
-            if (!valid) iy = at.hi[1];
-            const int k = pr >> 2, tt = pr & 3;
-            if (k < KY) {
-                hermite_gauss<NV>(displacement(iy, p.g.h, at.pos[1]), at, p.g.hnorm, numax, valid, v);
-#pragma unroll
-                for (int n = 0; n < MP; ++n) fy[((size_t)k * MT + (n >> 3)) * 32 + (n & 7) * 4 + tt] = v[n];
-                if (R) { fyr[2 * pr] = v[MP]; fyr[2 * pr + 1] = v[MP + R - 1]; }
-            }
-            // rows of the steps that pad the last group are never used in arithmetic; they point at a valid row
-            int jy = p.g.periodic[1] ? iy - floordiv(iy, Ny) * Ny : min(max(iy, 0), Ny - 1);
-            rowoff[((k / G) * 4 + tt) * G + (k % G)] = jy * Nx;      // [group][t][step in group]
-        } else if (it < ny_items + nx_items) {
-            const int j = it - ny_items;
+        if (it < nx_items) {
+            const int j = it;
             const int ix = xs0 + j;
             const bool valid = ix >= at.lo[0] && ix <= at.hi[0];
             hermite_gauss<NV>(displacement(ix, p.g.h, at.pos[0]), at, p.g.hnorm, numax, valid, v);
-            const int c = j / CW, r = j % CW;
-            int slot, tt;
-            if (!CPLX) { tt = r >> 2; slot = (c * 2 + (r & 1)) * 2 + ((r >> 1) & 1); }   // r = 4t + 2s + e
-            else       { tt = r >> 1; slot = c * 2 + (r & 1); }                           // r = 2t + s
+            const int kx = j / CWX, r = j % CWX, tt = r / EPL, e = r % EPL;      // column r of the step = EPL * t + e
 #pragma unroll
-            for (int n = 0; n < MP; ++n) fx[((size_t)slot * MT + (n >> 3)) * 32 + (n & 7) * 4 + tt] = v[n];
-            if (R) {
-                fxs[4 * j] = v[0]; fxs[4 * j + 1] = v[1]; fxs[4 * j + 2] = v[MP]; fxs[4 * j + 3] = v[MP + R - 1];
+            for (int n = 0; n < MP; ++n) fx[(((size_t)kx * EPL + e) * MT + (n >> 3)) * 32 + (n & 7) * 4 + tt] = v[n];
+            if (R) { fxr[2 * j] = v[MP]; fxr[2 * j + 1] = v[MP + R - 1]; }
+        } else if (it < nx_items + ny_items) {
+            const int pr = it - nx_items;                        // padded row slot
+            int iy = at.lo[1] + pr;
+            const bool valid = iy <= at.hi[1];
+            if (!valid) iy = at.hi[1];
+            hermite_gauss<NV>(displacement(iy, p.g.h, at.pos[1]), at, p.g.hnorm, numax, valid, v);
+            const int yb = pr >> 3, r = pr & 7, tt = r >> 1, s = r & 1;          // row r of the block = 2 t + s
+#pragma unroll
+            for (int n = 0; n < MP; ++n) fy[(((size_t)yb * 2 + s) * MT + (n >> 3)) * 32 + (n & 7) * 4 + tt] = v[n];
+            if (R) { fys[4 * pr] = v[0]; fys[4 * pr + 1] = v[1]; fys[4 * pr + 2] = v[MP]; fys[4 * pr + 3] = v[MP + R - 1]; }
+            const int my = p.g.periodic[1] ? floordiv(iy, Ny) : 0;
+            const int jy = p.g.periodic[1] ? iy - my * Ny : min(max(iy, 0), Ny - 1);
+            rowoff[pr] = jy * Nx;
+            if (CPLX) {
+                double sn = 0.0, cs = 1.0;
+                if (yphase) sincospi(2.0 * p.g.kfrac[1] * (double)my, &sn, &cs);
+                wy[2 * pr] = cs; wy[2 * pr + 1] = sn;
             }
         } else {
-            const int zi = it - ny_items - nx_items;
+            const int zi = it - nx_items - ny_items;
             const int iz = at.lo[2] + zi;
             hermite_gauss<NV>(displacement(iz, p.g.h, at.pos[2]), at, p.g.hnorm, numax, true, v);
 #pragma unroll
             for (int n = 0; n < NV; ++n) fz[(size_t)zi * NV + n] = v[n];
             if (CPLX) {
-                // phase of image m_z, times the overall y factor (phase of the last y segment)
+                // phase of image m_z, times the phase of the last x image
                 double ang = 0.0;
                 if (p.g.has_phase) {
                     if (p.g.periodic[2]) ang += p.g.kfrac[2] * (double)floordiv(iz, Nz);
-                    if (p.g.periodic[1]) ang += p.g.kfrac[1] * (double)floordiv(at.hi[1], Ny);
+                    if (p.g.periodic[0]) ang += p.g.kfrac[0] * (double)floordiv(at.hi[0], Nx);
                 }
                 double sn, cs;
                 sincospi(2.0 * ang, &sn, &cs);
@@ -179,25 +207,22 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
             }
         }
     }
+    // lane-span offsets of every x step (the steps that pad the last group repeat the last real step)
+    for (int it = tid; it < KXG * G * 4; it += blockDim.x) {
+        const int kx = it >> 2, tt = it & 3;
+        const int x0 = xs0 + CWX * min(kx, KX - 1) + EPL * tt;
+        const int off = p.g.periodic[0] ? x0 - floordiv(x0, Nx) * Nx : min(max(x0, 0), max(Nx - EPL, 0));
+        coloff[((kx / G) * 4 + tt) * G + (kx % G)] = off;
+    }
     if (CPLX && tid == 0) {
-        // x phases of the two possible images, and the y rotation exp(-2 pi i kfrac_y)
-        const int mlo = p.g.periodic[0] ? floordiv(at.lo[0], Nx) : 0;
-        for (int i = 0; i < 2; ++i) {
-            double sn, cs;
-            sincospi(2.0 * (p.g.has_phase && p.g.periodic[0] ? p.g.kfrac[0] * (double)(mlo + i) : 0.0), &sn, &cs);
-            phx[2 * i] = cs; phx[2 * i + 1] = sn;
-        }
         double sn, cs;
-        sincospi(-2.0 * p.g.kfrac[1], &sn, &cs);
-        phx[4] = cs; phx[5] = sn;
+        sincospi(-2.0 * p.g.kfrac[0], &sn, &cs);
+        phx[0] = cs; phx[1] = sn;
     }
     __syncthreads();
 
     const real_t* psi_b = reinterpret_cast<const real_t*>(p.psi) + (size_t)b * p.band_stride * P;
     const size_t plane = (size_t)Ny * Nx;
-    const bool vec = p.vec_ok != 0;
-    const int xB = CPLX ? (p.g.periodic[0] ? (floordiv(at.lo[0], Nx) + 1) * Nx : INT_MAX) : 0;
-    const bool xphase = CPLX && p.g.has_phase && p.g.periodic[0] && p.g.kfrac[0] != 0.0;
 
     // a5 accumulators: thread n owns coefficient(s) n, n + blockDim, ...
     double acc[NACC][P];
@@ -206,61 +231,60 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
     for (int j = 0; j < NACC; ++j) {
         const int n = tid + j * blockDim.x;
         const uint32_t pk = (n < p.g.nsho) ? p.nxyz[n] : 0u;
-        myt2[j] = t2_index<MT, R>((pk >> 8) & 255, pk & 255);
+        myt2[j] = t2_index<MT, R>(pk & 255, (pk >> 8) & 255);
         mynz[j] = (pk >> 16) & 255;
 #pragma unroll
         for (int pp = 0; pp < P; ++pp) acc[j][pp] = 0.0;
     }
 
-    // ---- a2 helpers: plane pointer, this lane's column pointer(s) of a chunk, one group of loads ----
+    // ---- a2 helpers: plane pointer, this lane's row pointer of a row block, one group of loads ----
     auto plane_ptr = [&](int zi) -> const real_t* {
         const int iz = at.lo[2] + zi;
         const int jz = p.g.periodic[2] ? iz - floordiv(iz, Nz) * Nz : iz;
         return psi_b + (size_t)jz * plane * P;
     };
-    auto col_ptrs = [&](const real_t* pzz, int c, const real_t*& c0, const real_t*& c1, bool& vv) {
-        const int ix0 = xs0 + c * CW + (CPLX ? q : 2 * q);
-        const int ix1 = ix0 + 1;
-        const int off0 = p.g.periodic[0] ? ix0 - floordiv(ix0, Nx) * Nx : min(max(ix0, 0), Nx - 1);
-        const int off1 = p.g.periodic[0] ? ix1 - floordiv(ix1, Nx) * Nx : min(max(ix1, 0), Nx - 1);
-        c0 = pzz + (size_t)off0 * P;
-        c1 = pzz + (size_t)off1 * P;
-        vv = vec && (CPLX || off1 == off0 + 1);
-    };
-    // G consecutive y steps (4 rows each) of one chunk: lane (q,t) reads row 4k+t, column(s) q / 2q, 2q+1
-    auto load_group = [&](double (&x0)[G], double (&x1)[G], const real_t* c0, const real_t* c1, bool vv, int kg) {
-        int r[G];
-        if (G == 4) {
-            const int4 r4 = *reinterpret_cast<const int4*>(rowoff + (kg * 4 + t) * G);
-            r[0] = r4.x; r[1] = r4.y; r[G - 2] = r4.z; r[G - 1] = r4.w;
-        } else {
-#pragma unroll
-            for (int j = 0; j < G; ++j) r[j] = rowoff[(kg * 4 + t) * G + j];
-        }
-#pragma unroll
-        for (int j = 0; j < G; ++j) {
-            const size_t ro = (size_t)r[j] * P;
-            if (CPLX) {
-                load2(c0 + ro, vec, x0[j], x1[j]);                            // (re, im) of one column
-            } else if (vv) {
-                load2(c0 + ro, true, x0[j], x1[j]);                           // two adjacent columns
+    auto row_ptr = [&](const real_t* pzz, int yb) -> const real_t* { return pzz + (size_t)rowoff[yb * 8 + q] * P; };
+    // G consecutive x steps of one row block: lane (q,t) reads columns EPL t .. EPL t + EPL - 1 of row q
+    auto load_group = [&](real_t (&raw)[G][RAW], const real_t* rp, int kg) {
+        if (fast) {
+            int co[G];
+            if (G == 2) {
+                const int2 c2 = *reinterpret_cast<const int2*>(coloff + (kg * 4 + t) * G);
+                co[0] = c2.x; co[G - 1] = c2.y;
             } else {
-                x0[j] = (double)__ldg(c0 + ro); x1[j] = (double)__ldg(c1 + ro);
+#pragma unroll
+                for (int j = 0; j < G; ++j) co[j] = coloff[(kg * 4 + t) * G + j];
+            }
+#pragma unroll
+            for (int j = 0; j < G; ++j) ldg256(rp + (size_t)co[j] * P, raw[j]);
+        } else {
+            // unaligned psi or Nx not a multiple of the lane span: element-wise loads, every column wrapped
+#pragma unroll
+            for (int j = 0; j < G; ++j) {
+                const int x0 = xs0 + CWX * min(kg * G + j, KX - 1) + EPL * t;
+#pragma unroll
+                for (int e = 0; e < EPL; ++e) {
+                    const int ix = x0 + e;
+                    const int off = p.g.periodic[0] ? ix - floordiv(ix, Nx) * Nx : min(max(ix, 0), Nx - 1);
+#pragma unroll
+                    for (int pp = 0; pp < P; ++pp) raw[j][e * P + pp] = __ldg(rp + (size_t)off * P + pp);
+                }
             }
         }
     };
 
-    // The load ring: while the G steps in cur0/cur1 are contracted, the next G steps are in flight; the
-    // ring runs on across chunk ends (over the x stage) and plane ends (over a5 and its barrier).
+    // The load ring: while the G steps in cur are contracted, the next G steps are in flight; the ring
+    // runs on across row-block ends (over the y stage) and plane ends (over a5 and its barrier).
     const int nrounds = (nzl + kProjWarps - 1) / kProjWarps;
-    double cur0[G], cur1[G];
-    const real_t *cp0 = psi_b, *cp1 = psi_b;     // column pointer(s) of the current chunk for this lane
-    bool cv = false;
+    real_t cur[G][RAW];
+    const real_t* rp = psi_b;                    // row pointer of the current row block for this lane
 #pragma unroll
-    for (int j = 0; j < G; ++j) cur0[j] = cur1[j] = 0.0;
+    for (int j = 0; j < G; ++j)
+#pragma unroll
+        for (int i = 0; i < RAW; ++i) cur[j][i] = (real_t)0;
     if (warp < nzl) {
-        col_ptrs(plane_ptr(warp), 0, cp0, cp1, cv);
-        load_group(cur0, cur1, cp0, cp1, cv, 0);
+        rp = row_ptr(plane_ptr(warp), 0);
+        load_group(cur, rp, 0);
     }
     for (int round = 0; round < nrounds; ++round) {
         const int zi = round * kProjWarps + warp;
@@ -269,41 +293,40 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
             const real_t* pz = plane_ptr(zi);
             const real_t* pzn = (zi + kProjWarps < nzl) ? plane_ptr(zi + kProjWarps) : pz;
 
-            // T2[part][ty][tx]: tile (1,1) can only hold ny+nx >= 16 > numax and is never needed
+            // T2[part][tx][ty]: tile (1,1) can only hold nx+ny >= 16 > numax and is never needed
             double T2[P][MT][MT][2];
 #pragma unroll
             for (int pp = 0; pp < P; ++pp)
 #pragma unroll
-                for (int ty = 0; ty < MT; ++ty)
+                for (int tx = 0; tx < MT; ++tx)
 #pragma unroll
-                    for (int tx = 0; tx < MT; ++tx) T2[pp][ty][tx][0] = T2[pp][ty][tx][1] = 0.0;
+                    for (int ty = 0; ty < MT; ++ty) T2[pp][tx][ty][0] = T2[pp][tx][ty][1] = 0.0;
             // R specials, per-lane partials: rs = T2[8][0], T2[8][1], T2[9][0]; cs = T2[q][8], T2[q][9]
             double rs[3][P], cs[2][P];
 #pragma unroll
             for (int pp = 0; pp < P; ++pp) { rs[0][pp] = rs[1][pp] = rs[2][pp] = 0.0; cs[0][pp] = cs[1][pp] = 0.0; }
 
-            for (int c = 0; c < XC; ++c) {
-                // where the ring goes after this chunk: the next chunk, or chunk 0 of this warp's next plane
-                const real_t *np0, *np1;
-                bool nv;
-                if (c + 1 < XC) col_ptrs(pz, c + 1, np0, np1, nv); else col_ptrs(pzn, 0, np0, np1, nv);
+            for (int yb = 0; yb < NYB; ++yb) {
+                // where the ring goes after this row block: the next block, or block 0 of this warp's next plane
+                const real_t* nrp = (yb + 1 < NYB) ? row_ptr(pz, yb + 1) : row_ptr(pzn, 0);
 
-                double C1[MT][2][2];   // [ny tile][e or re/im][s]
-                double ar[2][2];       // R rows: [ny = 8, 9][e or re/im], partial over this lane's row t
+                double C1[MT][2][2];   // [nx tile][re/im, or even/odd column for real data][s]
+                double ar[2][2];       // R rows: [nx = 8, 9][re/im], partial over this lane's columns
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) C1[mt][0][0] = C1[mt][0][1] = C1[mt][1][0] = C1[mt][1][1] = 0.0;
                 ar[0][0] = ar[0][1] = ar[1][0] = ar[1][1] = 0.0;
 
-                for (int kg = 0; kg < KG; ++kg) {
-                    const bool last = (kg == KG - 1);
-                    double n0[G], n1[G];
-                    load_group(n0, n1, last ? np0 : cp0, last ? np1 : cp1, last ? nv : cv, last ? 0 : kg + 1);
+                for (int kg = 0; kg < KXG; ++kg) {
+                    const bool last = (kg == KXG - 1);
+                    real_t nxt[G][RAW];
+                    load_group(nxt, last ? nrp : rp, last ? 0 : kg + 1);
 #pragma unroll
                     for (int j = 0; j < G; ++j) {
-                        const int k = kg * G + j;
-                        if (k < KY) {
-                            if (CPLX && k == krot) {
-                                const double cr = phx[4], ci = phx[5];
+                        const int kx = kg * G + j;
+                        if (kx < KX) {
+                            const bool rot = CPLX && kx == kx_rot;
+                            if (rot) {
+                                const double cr = phx[0], ci = phx[1];
 #pragma unroll
                                 for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
@@ -321,133 +344,118 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
                                     }
                                 }
                             }
-                            // ---- a3: y contraction, K = 4 rows ----
-                            const double v0 = cur0[j], v1 = cur1[j];
+                            // ---- a3: x contraction, EPL K steps of 4 columns ----
 #pragma unroll
-                            for (int mt = 0; mt < MT; ++mt) {
-                                const double afr = fy[((size_t)k * MT + mt) * 32 + lane];
-                                dmma(C1[mt][0][0], C1[mt][0][1], afr, v0);
-                                dmma(C1[mt][1][0], C1[mt][1][1], afr, v1);
-                            }
-                            if (R) {
-                                const double2 f = *reinterpret_cast<const double2*>(&fyr[2 * (4 * k + t)]);
-                                ar[0][0] = fma(f.x, v0, ar[0][0]); ar[0][1] = fma(f.x, v1, ar[0][1]);
-                                ar[1][0] = fma(f.y, v0, ar[1][0]); ar[1][1] = fma(f.y, v1, ar[1][1]);
+                            for (int e = 0; e < EPL; ++e) {
+                                double ve[P];
+#pragma unroll
+                                for (int pp = 0; pp < P; ++pp) ve[pp] = (double)cur[j][e * P + pp];
+                                if (rot && xs0 + CWX * kx + EPL * t + e < xB) {
+                                    // column of the first image inside the rotation step: same rotation for the value
+                                    const double cr = phx[0], ci = phx[1];
+                                    const double re = ve[0], im = ve[P - 1];
+                                    ve[0] = re * cr - im * ci;
+                                    ve[P - 1] = re * ci + im * cr;
+                                }
+#pragma unroll
+                                for (int mt = 0; mt < MT; ++mt) {
+                                    const double afr = fx[(((size_t)kx * EPL + e) * MT + mt) * 32 + lane];
+                                    if (CPLX) {
+                                        dmma(C1[mt][0][0], C1[mt][0][1], afr, ve[0]);
+                                        dmma(C1[mt][1][0], C1[mt][1][1], afr, ve[P - 1]);
+                                    } else {
+                                        dmma(C1[mt][e & 1][0], C1[mt][e & 1][1], afr, ve[0]);
+                                    }
+                                }
+                                if (R) {
+                                    const double2 f = *reinterpret_cast<const double2*>(&fxr[2 * (kx * CWX + EPL * t + e)]);
+#pragma unroll
+                                    for (int pp = 0; pp < P; ++pp) {
+                                        ar[0][pp] = fma(f.x, ve[pp], ar[0][pp]);
+                                        ar[1][pp] = fma(f.y, ve[pp], ar[1][pp]);
+                                    }
+                                }
                             }
                         }
                     }
 #pragma unroll
-                    for (int j = 0; j < G; ++j) { cur0[j] = n0[j]; cur1[j] = n1[j]; }
+                    for (int j = 0; j < G; ++j)
+#pragma unroll
+                        for (int i = 0; i < RAW; ++i) cur[j][i] = nxt[j][i];
                 }
 
-                // ---- Bloch phase of each column (complex only): rotate the accumulators ----
-                if (xphase) {
+                // real data: the even / odd column chains meet
+                if (!CPLX) {
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) { C1[mt][0][0] += C1[mt][1][0]; C1[mt][0][1] += C1[mt][1][1]; }
+                }
+                // ---- Bloch phase of each row (complex only): rotate the accumulators ----
+                if (yphase) {
 #pragma unroll
                     for (int s = 0; s < 2; ++s) {
-                        const int ix = xs0 + c * CW + 2 * t + s;
-                        const int im_ = (ix >= xB) ? 1 : 0;
-                        const double cr = phx[2 * im_], ci = phx[2 * im_ + 1];
+                        const double2 w = *reinterpret_cast<const double2*>(&wy[2 * (8 * yb + 2 * t + s)]);
 #pragma unroll
                         for (int mt = 0; mt < MT; ++mt) {
                             const double re = C1[mt][0][s], im = C1[mt][1][s];
-                            C1[mt][0][s] = re * cr - im * ci;
-                            C1[mt][1][s] = re * ci + im * cr;
+                            C1[mt][0][s] = re * w.x - im * w.y;
+                            C1[mt][1][s] = re * w.y + im * w.x;
                         }
                     }
                     if (R) {
-                        const int im_ = (xs0 + c * CW + q >= xB) ? 1 : 0;
-                        const double cr = phx[2 * im_], ci = phx[2 * im_ + 1];
+                        const double2 w = *reinterpret_cast<const double2*>(&wy[2 * (8 * yb + q)]);
 #pragma unroll
                         for (int i = 0; i < 2; ++i) {
                             const double re = ar[i][0], im = ar[i][1];
-                            ar[i][0] = re * cr - im * ci;
-                            ar[i][1] = re * ci + im * cr;
+                            ar[i][0] = re * w.x - im * w.y;
+                            ar[i][1] = re * w.y + im * w.x;
                         }
                     }
                 }
-                // ---- a4: x contraction; the a3 accumulators are the A fragments ----
-                if (!CPLX) {
+                // ---- a4: y contraction; the a3 accumulators are the A fragments (k = t <-> row 2t + s) ----
 #pragma unroll
-                    for (int e = 0; e < 2; ++e)
+                for (int s = 0; s < 2; ++s)
 #pragma unroll
-                        for (int s = 0; s < 2; ++s) {
-                            const int slot = (c * 2 + e) * 2 + s;
+                    for (int ty = 0; ty < MT; ++ty) {
+                        const double bfr = fy[(((size_t)yb * 2 + s) * MT + ty) * 32 + lane];
 #pragma unroll
-                            for (int tx = 0; tx < MT; ++tx) {
-                                const double bfr = fx[((size_t)slot * MT + tx) * 32 + lane];
+                        for (int tx = 0; tx < MT; ++tx)
+                            if (tx + ty < 2 || MT == 1) {
 #pragma unroll
-                                for (int ty = 0; ty < MT; ++ty)
-                                    if (ty + tx < 2 || MT == 1)
-                                        dmma(T2[0][ty][tx][0], T2[0][ty][tx][1], C1[ty][e][s], bfr);
+                                for (int pp = 0; pp < P; ++pp) dmma(T2[pp][tx][ty][0], T2[pp][tx][ty][1], C1[tx][pp][s], bfr);
                             }
-                        }
-                } else {
+                    }
+                if (R) {
+                    // rows nx = 8, 9 against phi_0, phi_1 of this lane's row; columns ny = 8, 9 against the a3
+                    // accumulators (rows nx = q; only q = 0, 1 are used)
+                    const double2 y0 = *reinterpret_cast<const double2*>(&fys[4 * (8 * yb + q)]);
+#pragma unroll
+                    for (int pp = 0; pp < P; ++pp) {
+                        rs[0][pp] = fma(ar[0][pp], y0.x, rs[0][pp]);
+                        rs[1][pp] = fma(ar[0][pp], y0.y, rs[1][pp]);
+                        rs[2][pp] = fma(ar[1][pp], y0.x, rs[2][pp]);
+                    }
 #pragma unroll
                     for (int s = 0; s < 2; ++s) {
-                        const int slot = c * 2 + s;
-#pragma unroll
-                        for (int tx = 0; tx < MT; ++tx) {
-                            const double bfr = fx[((size_t)slot * MT + tx) * 32 + lane];
-#pragma unroll
-                            for (int ty = 0; ty < MT; ++ty)
-                                if (ty + tx < 2 || MT == 1) {
-#pragma unroll
-                                    for (int pp = 0; pp < P; ++pp)
-                                        dmma(T2[pp][ty][tx][0], T2[pp][ty][tx][1], C1[ty][pp][s], bfr);
-                                }
-                        }
-                    }
-                }
-                if (R) {
-                    // rows ny = 8, 9 against phi_0, phi_1 of this lane's column(s); columns nx = 8, 9
-                    // against the a3 accumulators (rows ny = q; only q = 0, 1 are used)
-                    if (!CPLX) {
-                        const double* fr = fxs + 4 * (size_t)(c * CW + 2 * q);
-                        const double2 x0 = *reinterpret_cast<const double2*>(fr);
-                        const double2 x1 = *reinterpret_cast<const double2*>(fr + 4);
-                        rs[0][0] = fma(ar[0][0], x0.x, fma(ar[0][1], x1.x, rs[0][0]));
-                        rs[1][0] = fma(ar[0][0], x0.y, fma(ar[0][1], x1.y, rs[1][0]));
-                        rs[2][0] = fma(ar[1][0], x0.x, fma(ar[1][1], x1.x, rs[2][0]));
-#pragma unroll
-                        for (int e = 0; e < 2; ++e)
-#pragma unroll
-                            for (int s = 0; s < 2; ++s) {
-                                const double2 g =
-                                    *reinterpret_cast<const double2*>(fxs + 4 * (size_t)(c * CW + 4 * t + 2 * s + e) + 2);
-                                cs[0][0] = fma(C1[0][e][s], g.x, cs[0][0]);
-                                cs[1][0] = fma(C1[0][e][s], g.y, cs[1][0]);
-                            }
-                    } else {
-                        const double2 x0 = *reinterpret_cast<const double2*>(fxs + 4 * (size_t)(c * CW + q));
+                        const double2 g = *reinterpret_cast<const double2*>(&fys[4 * (8 * yb + 2 * t + s) + 2]);
 #pragma unroll
                         for (int pp = 0; pp < P; ++pp) {
-                            rs[0][pp] = fma(ar[0][pp], x0.x, rs[0][pp]);
-                            rs[1][pp] = fma(ar[0][pp], x0.y, rs[1][pp]);
-                            rs[2][pp] = fma(ar[1][pp], x0.x, rs[2][pp]);
-                        }
-#pragma unroll
-                        for (int s = 0; s < 2; ++s) {
-                            const double2 g = *reinterpret_cast<const double2*>(fxs + 4 * (size_t)(c * CW + 2 * t + s) + 2);
-#pragma unroll
-                            for (int pp = 0; pp < P; ++pp) {
-                                cs[0][pp] = fma(C1[0][pp][s], g.x, cs[0][pp]);
-                                cs[1][pp] = fma(C1[0][pp][s], g.y, cs[1][pp]);
-                            }
+                            cs[0][pp] = fma(C1[0][pp][s], g.x, cs[0][pp]);
+                            cs[1][pp] = fma(C1[0][pp][s], g.y, cs[1][pp]);
                         }
                     }
                 }
-                cp0 = np0; cp1 = np1; cv = nv;
+                rp = nrp;
             }
-            // plane result -> shared, [part][ny][nx] (+ the R specials)
+            // plane result -> shared, [part][nx][ny] (+ the R specials)
 #pragma unroll
             for (int pp = 0; pp < P; ++pp)
 #pragma unroll
-                for (int ty = 0; ty < MT; ++ty)
+                for (int tx = 0; tx < MT; ++tx)
 #pragma unroll
-                    for (int tx = 0; tx < MT; ++tx)
-                        if (ty + tx < 2 || MT == 1) {
-                            double2 o; o.x = T2[pp][ty][tx][0]; o.y = T2[pp][ty][tx][1];
-                            *reinterpret_cast<double2*>(&t2w[(size_t)pp * TS + (8 * ty + q) * MP + 8 * tx + 2 * t]) = o;
+                    for (int ty = 0; ty < MT; ++ty)
+                        if (tx + ty < 2 || MT == 1) {
+                            double2 o; o.x = T2[pp][tx][ty][0]; o.y = T2[pp][tx][ty][1];
+                            *reinterpret_cast<double2*>(&t2w[(size_t)pp * TS + (8 * tx + q) * MP + 8 * ty + 2 * t]) = o;
                         }
             if (R) {
 #pragma unroll
@@ -517,33 +525,30 @@ __global__ void sho_zero_empty_kernel(T* coeff, const int32_t* order, int first,
     (void)count;
 }
 
-
 template <int MT, int R, int DT>
 static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s)
 {
     using S = ProjSmem<MT, R, DT>;
     constexpr bool CPLX = Elem<DT>::cplx;
-    constexpr int CW = Elem<DT>::cw;
+    constexpr int EPL = S::EPL, CWX = S::CWX;
     ProjParams p;
     p.g = pl->g;
     p.psi = psi; p.coeff = coeff;
     p.atoms = pl->d_atoms; p.order = pl->d_order; p.nxyz = pl->d_nxyz;
     p.nbands = nbands;
     p.n_work_atoms = pl->n_nonempty;
-    p.ky_cap = (pl->max_n[1] + 3) / 4 + 2;
-    p.nxe_cap = ((pl->max_n[0] + 3 + CW - 1) / CW + 1) * (CPLX ? 2 : 4);
+    p.kx_cap = (pl->max_n[0] + 2 * (CWX - 1)) / CWX + 1;
+    p.yb_cap = (pl->max_n[1] + 7) / 8 + 1;
     p.nz_cap = pl->max_n[2] + 1;
     p.band_stride = (long long)pl->g.ng[0] * pl->g.ng[1] * pl->g.ng[2];
-    const size_t esz = elem_size(pl->dtype);
-    const size_t valign = CPLX ? esz : 2 * esz;      // bytes of one vector load
-    p.vec_ok = ((reinterpret_cast<uintptr_t>(psi) % valign) == 0) && (CPLX || (pl->g.ng[0] % 2 == 0));
-    const size_t smem = S::total_bytes(p.ky_cap, p.nxe_cap, p.nz_cap);
+    p.fast = ((reinterpret_cast<uintptr_t>(psi) % 32) == 0) && (pl->g.ng[0] % EPL == 0);
+    const size_t smem = S::total_bytes(p.kx_cap, p.yb_cap, p.nz_cap);
     if (smem > 227 * 1024) {
         set_error("sho_project: box of %d x %d x %d points needs %zu bytes of shared memory (> 227 KB)",
                   pl->max_n[0], pl->max_n[1], pl->max_n[2], smem);
         return SHO_ERR_UNSUPPORTED;
     }
-    auto kern = sho_project_kernel<MT, R, DT, (MT == 1 ? kProjG : 2)>;
+    auto kern = sho_project_kernel<MT, R, DT, kProjG>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(project)");
     const long long nblocks = (long long)pl->n_nonempty * nbands;
