@@ -7,23 +7,26 @@
 // list of (atom, periodic image) pairs whose box touches the tile, in ascending atom order, and finally
 // does ONE read-modify-write of the tile.  No atomics, bit-reproducible, psi traffic = read + write of
 // every touched tile exactly once.  Warp w owns z plane w of the tile (64 rows x 8 columns); two CTAs
-// share an SM so that one computes while the other samples its tables.
+// share an SM.
 //
-// Per batch of (tile, atom image) pairs, all three expansion stages run on DMMA.8x8x4:
-//   tables  (CTA-wide) the three 1D Hermite-Gauss tables of every pair are sampled on the fly (eq. (31),
-//           PAPER.md:283-286) into shared memory in MMA fragment order; the pair's coefficients
-//           c[a][b][:] are read once (coalesced), multiplied by the conjugate Bloch phase of the image
-//           and scattered into the A fragments of the z stage
-//   z       (CTA-wide, tasks spread over the warps)
-//           T2[z][(ny,nx)] = sum_nz c[n(nx,ny,nz)] phi_nz(z)         M = (ny,nx) pairs sorted by ny+nx, so
-//                                                                   that row tile mt needs only nz <=
-//                                                                   numax - s_min(mt); K = nz; N = 8 planes
-//   then every warp, for every pair of the batch that touches its plane:
-//   x       T1[x][ny]  = sum_nx phi_nx(x) T2[z][(ny,nx)]             M = x, K = nx, N = ny
-//   y       psi[y][x] += sum_ny phi_ny(y) T1[x][ny]                  M = y, K = ny, N = x
-// The accumulator fragment of the x stage is exactly the B fragment of the y stage when column 2t+s of
-// the x stage's N tile is assigned ny = 8 nt + 4 s + t: the contracted index is then cut in K steps of
-// four consecutive ny, so only ceil((numax+1)/4) steps are issued.
+// The pair list is consumed in groups of NG pairs by a software pipeline with ONE barrier per step; in
+// step s every warp runs, back to back and without waiting for the other warps,
+//   E(s+1)  cp.async of the 96-byte records of the next group (atom parameters included: no pointer chase)
+//   C(s)    issue the global loads of the group's coefficients c[a][b][:] (consumed at the end of the step)
+//   XY(s-2) the x and y stages of the group whose tables and T2 are complete, on its own z plane:
+//             x   T1[x][ny]  = sum_nx phi_nx(x) T2[z][(ny,nx)]       M = x, K = nx, N = ny
+//             y   psi[y][x] += sum_ny phi_ny(y) T1[x][ny]            M = y, K = ny, N = x
+//           The accumulator fragment of the x stage is exactly the B fragment of the y stage when column
+//           2t+s of the x stage's N tile is assigned ny = 8 nt + 4 s + t.
+//   Z(s-1)  its share of the z stage of the previous group
+//             T2[z][(ny,nx)] = sum_nz c[n(nx,ny,nz)] phi_nz(z)       M = (ny,nx) pairs sorted by ny+nx, so that
+//                                                                   row tile mt needs only nz <= numax -
+//                                                                   s_min(mt); K = nz; N = 8 planes
+//   T(s)    its share of the group's three 1D Hermite-Gauss tables, sampled on the fly (eq. (31),
+//           PAPER.md:283-286) into shared memory in MMA fragment order, and the scatter of the (now arrived)
+//           coefficients, times the conjugate Bloch phase of the image, into the A fragments of the z stage
+// so the latency-bound stages (E, C, T) of one warp overlap the tensor-core stages of the others.  All
+// three expansion stages run on DMMA.8x8x4.  Ring depths: x/y tables 3, everything else 2.
 #include "sho_device.cuh"
 
 namespace sho {
@@ -33,32 +36,39 @@ struct AddParams {
     AddZTiles zt;
     const void* coeff;
     void* psi;
-    const AtomDev* atoms;
     const int32_t* tile_ptr;
     const AddEntry* tile_ent;
     const int32_t* tile_list;
     const uint16_t* cainv;
+    const uint16_t* t2pos;
     int32_t n_tile_list;
     int32_t nbands;
     int32_t ntile0, ntile1;
     int32_t vec_ok;
-    int32_t batch;             // pairs per batch (shared-memory slots)
-    int32_t npp;               // row stride of T2 (doubles): 8 nmt + 2, = 2 mod 8 and != 0 mod 16 (bank spread)
-    int32_t slot;              // doubles per pair slot
+    int32_t ng;                // pairs per pipeline step (NG)
+    int32_t npp;               // plane stride of T2 (doubles): 8 nmt + 2; column 8 nmt holds zeros
     long long band_stride;
 };
 
 constexpr int kAddPoints = kAddTY + kAddTX + kAddTZ;    // 1D sample points per pair: 8 y blocks, 1 x block, 1 z block
 
-// slot layout (doubles): [F: 10 blocks x KQ x 32][CA: nblk x P x 32][T2: P x 8 x npp][head: 2]
+// shared-memory carve-up (doubles): [FXY: 3 NG x 9 KQ 32][FZ: 2 NG x KQ 32][CA: 2 NG x nblk P 32][T2: 2 NG x P 8 npp]
+// then [ENT: 2 NG records][META: 3 NG int32][ZPOS: 8 nmt uint16]
 template <int KQ, int DT>
 struct AddSmem {
     static constexpr int P = Elem<DT>::cplx ? 2 : 1;
-    static constexpr int F = (kAddPoints / 8) * KQ * 32;
-    static __host__ __device__ int ca(int) { return F; }
-    static __host__ __device__ int t2(int nblk) { return F + nblk * P * 32; }
-    static __host__ __device__ int head(int nblk, int npp) { return t2(nblk) + P * kAddTZ * npp; }
-    static __host__ __device__ int slot_doubles(int nblk, int npp) { return head(nblk, npp) + 2; }
+    static constexpr int FXYS = 9 * KQ * 32;
+    static constexpr int FZS = KQ * 32;
+    static constexpr int CPT = (KQ == 4) ? 4 : 2;            // coefficients a thread holds in flight per step
+    static __host__ __device__ int cas(int nblk) { return nblk * P * 32; }
+    static __host__ __device__ int t2s(int npp) { return P * kAddTZ * npp; }
+    static __host__ __device__ size_t bytes(int ng, int nblk, int nmt)
+    {
+        const int npp = 8 * nmt + 2;
+        size_t b = 8 * (size_t)ng * (3 * FXYS + 2 * FZS + 2 * cas(nblk) + 2 * t2s(npp));
+        b += (size_t)2 * ng * sizeof(AddEntry) + (size_t)3 * ng * 4 + (size_t)8 * nmt * 2;
+        return (b + 15) & ~(size_t)15;
+    }
 };
 
 // phi_0..phi_{NV-1} as in sho_device.cuh::hermite_gauss, from the scalars of one atom
@@ -78,6 +88,37 @@ __device__ __forceinline__ void hermite_gauss_s(double u, double inv_sigma, doub
     }
 }
 
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
+{
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+
+// coefficient loads that stay where they are issued (start of the step), read-only path
+__device__ __forceinline__ void ldg_pinned(const double* p, bool vec, double& re, double& im)
+{
+    if (vec) asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(re), "=d"(im) : "l"(p));
+    else { asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(re) : "l"(p)); asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(im) : "l"(p + 1)); }
+}
+__device__ __forceinline__ void ldg_pinned(const float* p, bool vec, double& re, double& im)
+{
+    float a, b;
+    if (vec) asm volatile("ld.global.nc.v2.f32 {%0,%1}, [%2];" : "=f"(a), "=f"(b) : "l"(p));
+    else { asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(a) : "l"(p)); asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(b) : "l"(p + 1)); }
+    re = (double)a; im = (double)b;
+}
+__device__ __forceinline__ void ldg_pinned(const double* p, double& re)
+{
+    asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(re) : "l"(p));
+}
+__device__ __forceinline__ void ldg_pinned(const float* p, double& re)
+{
+    float a;
+    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(a) : "l"(p));
+    re = (double)a;
+}
+
 template <int KQ, int DT>
 __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddParams p)
 {
@@ -89,13 +130,22 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
     constexpr int NV = 4 * KQ;                 // sampled functions per point (numax + 1 rounded up to 4)
     constexpr int NT = (KQ + 1) / 2;           // ny tiles of 8 in the x stage
     constexpr int NYT = kAddTY / 8;
+    constexpr int FXYS = S::FXYS, FZS = S::FZS, CPT = S::CPT;
+    constexpr int NTHR = kAddWarps * 32;
     static_assert(kAddTX == 8 && kAddTZ == 8 && kAddWarps == 8, "one 8x8 MMA block per x / z extent");
 
     extern __shared__ __align__(16) double smem[];
     const int nsho = p.g.nsho;
-    const int SLOT = p.slot;
+    const int NG = p.ng;
     const int nblk = p.zt.nblk, nmt = p.zt.nmt, npp = p.npp;
-    const int CA = S::ca(nblk), T2 = S::t2(nblk), HEAD = S::head(nblk, npp);
+    const int CAS = S::cas(nblk), T2S = S::t2s(npp);
+    double* FXY = smem;                                   // [3][NG][FXYS]  y blocks 0..7, x block 8
+    double* FZ = FXY + (size_t)3 * NG * FXYS;             // [2][NG][FZS]
+    double* CA = FZ + (size_t)2 * NG * FZS;               // [2][NG][CAS]   A fragments of the z stage
+    double* T2 = CA + (size_t)2 * NG * CAS;               // [2][NG][T2S]
+    AddEntry* ENT = reinterpret_cast<AddEntry*>(T2 + (size_t)2 * NG * T2S);      // [2][NG]
+    int32_t* META = reinterpret_cast<int32_t*>(ENT + 2 * NG);                    // [3][NG] zmask | ytlo << 8 | ythi << 16
+    uint16_t* ZPOS = reinterpret_cast<uint16_t*>(META + 3 * NG);                 // [8 nmt] T2 column of z-stage row
 
     const int tid = threadIdx.x, lane = tid & 31, zl = tid >> 5;
     const int q = lane >> 2, t = lane & 3;
@@ -107,10 +157,24 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
     const int Nx = p.g.ng[0], Ny = p.g.ng[1], Nz = p.g.ng[2];
     const int numax = p.g.numax;
     const int ebeg = p.tile_ptr[tile], eend = p.tile_ptr[tile + 1];
-    const int NB = p.batch;
+    const int npairs = eend - ebeg;
+    const int nG = (npairs + NG - 1) / NG;
 
-    // zero the slots once: the padding entries of the z-stage A fragments and the zero column of T2 stay zero
-    for (int i = tid; i < NB * SLOT; i += blockDim.x) smem[i] = 0.0;
+    // E: records of group g -> ENT[g & 1], six 16-byte pieces each
+    auto fetch_entries = [&](int g) {
+        if (tid < NG * 6) {
+            const int i = tid / 6, piece = tid - 6 * i;
+            const int e = g * NG + i;
+            if (e < npairs)
+                cp_async16(reinterpret_cast<char*>(ENT + (g & 1) * NG + i) + 16 * piece,
+                           reinterpret_cast<const char*>(p.tile_ent + ebeg + e) + 16 * piece);
+        }
+    };
+    fetch_entries(0);
+
+    // zero CA and T2 once: the padding entries of the z-stage A fragments and the zero column of T2 stay zero
+    for (int i = tid; i < 2 * NG * (CAS + T2S); i += NTHR) CA[i] = 0.0;
+    for (int i = tid; i < 8 * nmt; i += NTHR) ZPOS[i] = p.t2pos[256 + i];
 
     double D[NYT][P][2];
 #pragma unroll
@@ -124,124 +188,163 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
 #pragma unroll
     for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
-        for (int ks = 0; ks < KQ; ++ks) {
-            const int ny = 8 * nt + 4 * (q & 1) + (q >> 1), nx = 4 * ks + t, s = ny + nx;
-            t2off[nt][ks] = (s <= numax) ? (s * (s + 1)) / 2 + nx : 8 * nmt;
-        }
+        for (int ks = 0; ks < KQ; ++ks) t2off[nt][ks] = p.t2pos[16 * (8 * nt + 4 * (q & 1) + (q >> 1)) + 4 * ks + t];
 
-    const real_t* cbase = reinterpret_cast<const real_t*>(p.coeff);
+    // this thread's share of a group's coefficients: slot k = coefficient cn[k] of pair ci[k] -> CA offset co[k]
+    int ci[CPT], cn[CPT], co[CPT];
+#pragma unroll
+    for (int k = 0; k < CPT; ++k) {
+        const int idx = tid + k * NTHR;
+        ci[k] = -1; cn[k] = 0; co[k] = 0;
+        if (idx < NG * nsho) {
+            ci[k] = idx / nsho;
+            cn[k] = idx - ci[k] * nsho;
+            const int o = p.cainv[cn[k]];
+            co[k] = ci[k] * CAS + (o >> 5) * (32 * P) + (o & 31);
+        }
+    }
 
-    for (int e0 = ebeg; e0 < eend; e0 += NB) {
-        const int nb = min(NB, eend - e0);
-        __syncthreads();                                        // the previous batch's tables are no longer read
-        // ---------------- tables: 1D functions (step a1) in fragment order ----------------
-        for (int it = tid; it < nb * kAddPoints; it += blockDim.x) {
-            const int i = it / kAddPoints, r = it - i * kAddPoints;
-            const AddEntry* en = p.tile_ent + e0 + i;
-            const AtomDev* at = p.atoms + en->atom;
-            const int d = r < kAddTY ? 1 : (r < kAddTY + kAddTX ? 0 : 2);
-            const int N = p.g.ng[d];
-            const int j = (d == 1 ? jy0 + r : (d == 0 ? jx0 : jz0) + (r & 7));
-            const int iu = j + (int)en->m[d] * N;
-            const bool valid = j < N && iu >= at->lo[d] && iu <= at->hi[d];
-            double v[NV];
-            if (valid) {
-                hermite_gauss_s<NV>(displacement(iu, p.g.h, at->pos[d]), at->inv_sigma, at->pref, p.g.hnorm, numax, v);
-            } else {
+    const real_t* cbase = reinterpret_cast<const real_t*>(p.coeff) + (size_t)b * nsho * P;
+    const size_t catom = (size_t)p.nbands * nsho * P;
+    const bool cvec = p.vec_ok != 0;
+
+    cp_async_wait_all();
+    __syncthreads();
+
+    int r3 = 0;                                             // s mod 3
+    for (int s = 0; s < nG + 2; ++s) {
+        const int r2 = s & 1;
+        const int r3m2 = (r3 == 0) ? 1 : (r3 == 1 ? 2 : 0);  // (s - 2) mod 3
+        // ---------------- E(s+1) ----------------
+        if (s + 1 < nG) fetch_entries(s + 1);
+        // ---------------- C(s): issue the coefficient loads ----------------
+        double creg[CPT][P];
+        if (s < nG) {
 #pragma unroll
-                for (int n = 0; n < NV; ++n) v[n] = 0.0;
-            }
-            // block r >> 3 (y: 0..7, x: 8, z: 9), point r & 7: element [k = n & 3] of K step n >> 2
-            double* dst = smem + (size_t)i * SLOT + ((r >> 3) * KQ) * 32 + (r & 7) * 4;
+            for (int k = 0; k < CPT; ++k) {
 #pragma unroll
-            for (int kk = 0; kk < KQ; ++kk) {
-                double2 a, c;
-                a.x = v[4 * kk]; a.y = v[4 * kk + 1]; c.x = v[4 * kk + 2]; c.y = v[4 * kk + 3];
-                *reinterpret_cast<double2*>(dst + kk * 32) = a;
-                *reinterpret_cast<double2*>(dst + kk * 32 + 2) = c;
+                for (int pp = 0; pp < P; ++pp) creg[k][pp] = 0.0;
+                if (ci[k] >= 0 && s * NG + ci[k] < npairs) {
+                    const real_t* c = cbase + (size_t)ENT[r2 * NG + ci[k]].atom * catom + (size_t)cn[k] * P;
+                    if (CPLX) ldg_pinned(c, cvec, creg[k][0], creg[k][P - 1]);
+                    else ldg_pinned(c, creg[k][0]);
+                }
             }
         }
-        if (tid < nb) {
-            const AddEntry* en = p.tile_ent + e0 + tid;
-            int32_t* meta = reinterpret_cast<int32_t*>(smem + (size_t)tid * SLOT + HEAD);
-            meta[0] = en->ytlo; meta[1] = en->ythi; meta[2] = en->zmask; meta[3] = en->atom;
+        // ---------------- XY(s-2): every warp on its own plane ----------------
+        if (s >= 2) {
+            for (int i = 0; i < NG; ++i) {
+                const int meta = META[r3m2 * NG + i];
+                if (!((meta >> zl) & 1)) continue;
+                const int ytlo = (meta >> 8) & 0xff, ythi = (meta >> 16) & 0xff;
+                const double* fxy = FXY + (size_t)(r3m2 * NG + i) * FXYS + lane;
+                const double* t2p = T2 + (size_t)(r2 * NG + i) * T2S + (size_t)zl * npp;
+
+                double D1[NT][P][2];
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+                    for (int pp = 0; pp < P; ++pp) D1[nt][pp][0] = D1[nt][pp][1] = 0.0;
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+                    for (int ks = 0; ks < KQ; ++ks)
+                        if (8 * nt + 4 * ks <= numax) {                     // warp-uniform: the block holds some ny+nx <= numax
+                            const double a = fxy[(8 * KQ + ks) * 32];
+#pragma unroll
+                            for (int pp = 0; pp < P; ++pp)
+                                dmma(D1[nt][pp][0], D1[nt][pp][1], a, t2p[(size_t)pp * kAddTZ * npp + t2off[nt][ks]]);
+                        }
+#pragma unroll
+                for (int yt = 0; yt < NYT; ++yt)
+                    if (yt >= ytlo && yt <= ythi) {
+#pragma unroll
+                        for (int kk = 0; kk < KQ; ++kk) {
+                            const double a = fxy[(yt * KQ + kk) * 32];
+#pragma unroll
+                            for (int pp = 0; pp < P; ++pp) dmma(D[yt][pp][0], D[yt][pp][1], a, D1[kk >> 1][pp][kk & 1]);
+                        }
+                    }
+            }
         }
-        // coefficients of the batch: coalesced read, conjugate image phase, scatter into the z-stage A fragments
-        for (int i = 0; i < nb; ++i) {
-            const AddEntry* en = p.tile_ent + e0 + i;
-            const real_t* c = cbase + ((size_t)en->atom * p.nbands + b) * nsho * P;
-            double* ca = smem + (size_t)i * SLOT + CA;
-            const double wr = en->wr, wi = en->wi;
-            for (int n = tid; n < nsho; n += blockDim.x) {
-                const int o = p.cainv[n];
-                double* dst = ca + (o >> 5) * (32 * P) + (o & 31);
-                if (!CPLX) {
-                    dst[0] = (double)__ldg(c + n);
+        // ---------------- Z(s-1): T2[z][(ny,nx)] for the 8 planes of the tile ----------------
+        if (s >= 1 && s - 1 < nG) {
+            const int r2m1 = r2 ^ 1;
+            const int cnt = min(NG, npairs - (s - 1) * NG);
+            for (int task = zl; task < cnt * nmt; task += kAddWarps) {
+                const int i = task / nmt, mt = task - i * nmt;
+                const double* fz = FZ + (size_t)(r2m1 * NG + i) * FZS + lane;
+                const double* ap = CA + (size_t)(r2m1 * NG + i) * CAS + (size_t)p.zt.blk0[mt] * (32 * P) + lane;
+                const int nks = p.zt.nks[mt];
+                double d[P][2];
+#pragma unroll
+                for (int pp = 0; pp < P; ++pp) d[pp][0] = d[pp][1] = 0.0;
+                for (int ks = 0; ks < nks; ++ks) {
+                    const double bfr = fz[ks * 32];                            // B[k = nz][col = plane]
+#pragma unroll
+                    for (int pp = 0; pp < P; ++pp) dmma(d[pp][0], d[pp][1], ap[(ks * P + pp) * 32], bfr);
+                }
+                double* o = T2 + (size_t)(r2m1 * NG + i) * T2S + (size_t)(2 * t) * npp + ZPOS[8 * mt + q];
+#pragma unroll
+                for (int pp = 0; pp < P; ++pp) {
+                    o[(size_t)pp * kAddTZ * npp] = d[pp][0];
+                    o[(size_t)pp * kAddTZ * npp + npp] = d[pp][1];
+                }
+            }
+        }
+        // ---------------- T(s): 1D functions (step a1) in fragment order; scatter of C(s) ----------------
+        if (s < nG) {
+            for (int it = tid; it < NG * kAddPoints; it += NTHR) {
+                const int i = it / kAddPoints, r = it - i * kAddPoints;
+                if (s * NG + i >= npairs) break;
+                const AddEntry* en = ENT + r2 * NG + i;
+                const int d = r < kAddTY ? 1 : (r < kAddTY + kAddTX ? 0 : 2);
+                const int N = p.g.ng[d];
+                const int j = (d == 1 ? jy0 + r : (d == 0 ? jx0 : jz0) + (r & 7));
+                const int iu = j + (int)en->m[d] * N;
+                const bool valid = j < N && iu >= en->lo[d] && iu <= en->hi[d];
+                double v[NV];
+                if (valid) {
+                    hermite_gauss_s<NV>(displacement(iu, p.g.h, en->pos[d]), en->inv_sigma, en->pref, p.g.hnorm, numax, v);
                 } else {
-                    double re, im;
-                    load2(c + 2 * (size_t)n, p.vec_ok != 0, re, im);
-                    dst[0] = re * wr - im * wi;
-                    dst[32] = re * wi + im * wr;
+#pragma unroll
+                    for (int n = 0; n < NV; ++n) v[n] = 0.0;
+                }
+                // block r >> 3 (y: 0..7, x: 8, z: own ring), point r & 7: element [k = n & 3] of K step n >> 2
+                double* dst = (d == 2) ? FZ + (size_t)(r2 * NG + i) * FZS + (r & 7) * 4
+                                       : FXY + (size_t)(r3 * NG + i) * FXYS + ((r >> 3) * KQ) * 32 + (r & 7) * 4;
+#pragma unroll
+                for (int kk = 0; kk < KQ; ++kk) {
+                    double2 a, c;
+                    a.x = v[4 * kk]; a.y = v[4 * kk + 1]; c.x = v[4 * kk + 2]; c.y = v[4 * kk + 3];
+                    *reinterpret_cast<double2*>(dst + kk * 32) = a;
+                    *reinterpret_cast<double2*>(dst + kk * 32 + 2) = c;
                 }
             }
-        }
-        __syncthreads();
-        // ---------------- z stage: T2[z][(ny,nx)] for the 8 planes of the tile ----------------
-        for (int task = zl; task < nb * nmt; task += kAddWarps) {
-            const int i = task / nmt, mt = task - i * nmt;
-            double* slot = smem + (size_t)i * SLOT;
-            const int blk0 = p.zt.blk0[mt], nks = p.zt.nks[mt];
-            double d[P][2];
-#pragma unroll
-            for (int pp = 0; pp < P; ++pp) d[pp][0] = d[pp][1] = 0.0;
-            for (int ks = 0; ks < nks; ++ks) {
-                const double bfr = slot[(9 * KQ + ks) * 32 + lane];            // B[k = nz][col = plane]
-                const double* ap = slot + CA + (size_t)(blk0 + ks) * (32 * P) + lane;
-#pragma unroll
-                for (int pp = 0; pp < P; ++pp) dmma(d[pp][0], d[pp][1], ap[32 * pp], bfr);
+            if (tid < NG) {
+                const AddEntry* en = ENT + r2 * NG + tid;
+                META[r3 * NG + tid] = (s * NG + tid < npairs)
+                                          ? ((int)en->zmask | ((int)en->ytlo << 8) | ((int)en->ythi << 16)) : 0;
             }
+            // coefficients of the group: conjugate image phase, scatter into the z-stage A fragments
+            double* ca = CA + (size_t)r2 * NG * CAS;
 #pragma unroll
-            for (int pp = 0; pp < P; ++pp) {
-                double* o = slot + T2 + ((size_t)pp * kAddTZ + 2 * t) * npp + 8 * mt + q;
-                o[0] = d[pp][0];
-                o[npp] = d[pp][1];
-            }
-        }
-        __syncthreads();
-        // ---------------- x and y stages: every warp on its own plane ----------------
-        for (int i = 0; i < nb; ++i) {
-            const double* slot = smem + (size_t)i * SLOT;
-            const int32_t* meta = reinterpret_cast<const int32_t*>(slot + HEAD);
-            const int ytlo = meta[0], ythi = meta[1];
-            if (!((meta[2] >> zl) & 1)) continue;
-            const double* t2p = slot + T2 + (size_t)zl * npp;
-
-            double D1[NT][P][2];
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-                for (int pp = 0; pp < P; ++pp) D1[nt][pp][0] = D1[nt][pp][1] = 0.0;
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-                for (int ks = 0; ks < KQ; ++ks)
-                    if (8 * nt + 4 * ks <= numax) {                     // warp-uniform: the block holds some ny+nx <= numax
-                        const double a = slot[(8 * KQ + ks) * 32 + lane];
-#pragma unroll
-                        for (int pp = 0; pp < P; ++pp)
-                            dmma(D1[nt][pp][0], D1[nt][pp][1], a, t2p[(size_t)pp * kAddTZ * npp + t2off[nt][ks]]);
-                    }
-#pragma unroll
-            for (int yt = 0; yt < NYT; ++yt)
-                if (yt >= ytlo && yt <= ythi) {
-#pragma unroll
-                    for (int kk = 0; kk < KQ; ++kk) {
-                        const double a = slot[(yt * KQ + kk) * 32 + lane];
-#pragma unroll
-                        for (int pp = 0; pp < P; ++pp) dmma(D[yt][pp][0], D[yt][pp][1], a, D1[kk >> 1][pp][kk & 1]);
+            for (int k = 0; k < CPT; ++k)
+                if (ci[k] >= 0 && s * NG + ci[k] < npairs) {
+                    if (!CPLX) {
+                        ca[co[k]] = creg[k][0];
+                    } else {
+                        const AddEntry* en = ENT + r2 * NG + ci[k];
+                        const double wr = en->wr, wi = en->wi;
+                        const double re = creg[k][0], im = creg[k][P - 1];
+                        ca[co[k]] = re * wr - im * wi;
+                        ca[co[k] + 32] = re * wi + im * wr;
                     }
                 }
         }
+        cp_async_wait_all();
+        __syncthreads();
+        r3 = (r3 == 2) ? 0 : r3 + 1;
     }
 
     // ---------------- one read-modify-write of the owned tile ----------------
@@ -292,9 +395,8 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
     p.g = pl->g;
     p.zt = pl->ztiles;
     p.coeff = coeff; p.psi = psi;
-    p.atoms = pl->d_atoms;
     p.tile_ptr = pl->d_tile_ptr; p.tile_ent = pl->d_tile_ent; p.tile_list = pl->d_tile_list;
-    p.cainv = pl->d_cainv;
+    p.cainv = pl->d_cainv; p.t2pos = pl->d_t2pos;
     p.n_tile_list = pl->n_tile_list;
     p.nbands = nbands;
     p.ntile0 = pl->ntile[0]; p.ntile1 = pl->ntile[1];
@@ -304,11 +406,17 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
     p.vec_ok = ((reinterpret_cast<uintptr_t>(psi) % valign) == 0) && (CPLX || (pl->g.ng[0] % 2 == 0));
     if (CPLX && (reinterpret_cast<uintptr_t>(coeff) % esz) != 0) p.vec_ok = 0;
     p.npp = 8 * pl->ztiles.nmt + 2;
-    p.slot = S::slot_doubles(pl->ztiles.nblk, p.npp);
-    const size_t slot_bytes = (size_t)p.slot * 8;
-    const size_t budget = 112 * 1024;                        // two CTAs per SM
-    p.batch = (int)std::max<size_t>(1, std::min<size_t>(16, budget / slot_bytes));
-    const size_t smem = slot_bytes * p.batch;
+    // pairs per pipeline step: as many as fit two CTAs per SM and CPT coefficients per thread (at most 4)
+    const size_t budget = 112 * 1024;
+    int ng = 1;
+    while (ng < 4 && S::bytes(ng + 1, pl->ztiles.nblk, pl->ztiles.nmt) <= budget &&
+           (ng + 1) * pl->g.nsho <= S::CPT * kAddWarps * 32) ++ng;
+    p.ng = ng;
+    const size_t smem = S::bytes(ng, pl->ztiles.nblk, pl->ztiles.nmt);
+    if (smem > 227 * 1024 || pl->g.nsho > S::CPT * kAddWarps * 32) {
+        set_error("sho_add: numax = %d needs %zu bytes of shared memory (> 227 KB)", pl->g.numax, smem);
+        return SHO_ERR_UNSUPPORTED;
+    }
     auto kern = sho_add_kernel<KQ, DT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(add)");

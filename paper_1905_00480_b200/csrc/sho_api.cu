@@ -52,9 +52,9 @@ static sho_status upload(T** dst, const std::vector<T>& src, const char* what)
 static void plan_free_device(sho_plan* p)
 {
     cudaFree(p->d_atoms); cudaFree(p->d_order); cudaFree(p->d_nxyz);
-    cudaFree(p->d_tile_ptr); cudaFree(p->d_tile_ent); cudaFree(p->d_tile_list); cudaFree(p->d_cainv);
+    cudaFree(p->d_tile_ptr); cudaFree(p->d_tile_ent); cudaFree(p->d_tile_list); cudaFree(p->d_cainv); cudaFree(p->d_t2pos);
     cudaFree(p->ws_psi); cudaFree(p->ws_c);
-    p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr; p->d_cainv = nullptr;
+    p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr;
     p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr;
     p->ws_psi = nullptr; p->ws_c = nullptr;
 }
@@ -122,7 +122,7 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
     sho_plan* p = new (std::nothrow) sho_plan();
     if (!p) { set_error("sho_plan_create: host allocation failed"); return SHO_ERR_OOM; }
     p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr;
-    p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr; p->d_cainv = nullptr;
+    p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr;
     p->ws_psi = nullptr; p->ws_c = nullptr; p->ws_psi_bytes = 0; p->ws_c_bytes = 0;
     p->rcut_sigma = rcut_sigma;
     p->dtype = dtype;
@@ -269,6 +269,8 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
                                 AddEntry e;
                                 std::memset(&e, 0, sizeof(e));
                                 e.atom = a; e.m[0] = (int16_t)x.m; e.m[1] = (int16_t)y.m; e.m[2] = (int16_t)z.m;
+                                for (int d = 0; d < 3; ++d) { e.pos[d] = at.pos[d]; e.lo[d] = at.lo[d]; e.hi[d] = at.hi[d]; }
+                                e.inv_sigma = at.inv_sigma; e.pref = at.pref;
                                 // overlap of the box with the tile, in the units the warps can skip
                                 const int oy = y.tile * kAddTY + y.m * g.ng[1], oz = z.tile * kAddTZ + z.m * g.ng[2];
                                 const int ylast = std::min(kAddTY, g.ng[1] - y.tile * kAddTY) - 1;
@@ -325,6 +327,27 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
                 }
     }
 
+    // ---- columns of the add's T2[z][column]: the x stage reads pair (ny,nx) as the B fragment of block
+    // (nt,ks) with ny = 8 nt + 4 (q & 1) + (q >> 1), nx = 4 ks + t on lane 4 q + t; the pairs of a block
+    // get consecutive columns in lane order, so that a warp's read is one contiguous, conflict-free run
+    std::vector<uint16_t> t2pos((size_t)256 + 8 * p->ztiles.nmt, 0);
+    {
+        const int zero_col = 8 * p->ztiles.nmt;
+        for (auto& v : t2pos) v = (uint16_t)zero_col;
+        const int KQ = (numax + 4) >> 2, NT = (KQ + 1) / 2;
+        int col = 0;
+        for (int nt = 0; nt < NT; ++nt)
+            for (int ks = 0; ks < KQ; ++ks)
+                for (int lane = 0; lane < 32; ++lane) {
+                    const int q = lane >> 2, t = lane & 3;
+                    const int ny = 8 * nt + 4 * (q & 1) + (q >> 1), nx = 4 * ks + t;
+                    if (ny + nx <= numax) t2pos[(size_t)16 * ny + nx] = (uint16_t)col++;
+                }
+        // z-stage row 8 mt + q = pair index s (s + 1) / 2 + nx with s = ny + nx (rows past the last pair hold zeros)
+        for (int s = 0; s <= numax; ++s)
+            for (int nx = 0; nx <= s; ++nx) t2pos[(size_t)256 + s * (s + 1) / 2 + nx] = t2pos[(size_t)16 * (s - nx) + nx];
+    }
+
     // ---- device mirrors ----
     cudaError_t e = cudaGetDevice(&p->device);
     if (e != cudaSuccess) { sho_status s = cuda_fail(e, "sho_plan_create: cudaGetDevice (no CUDA device?)"); delete p; return s; }
@@ -335,7 +358,8 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
         (st = upload(&p->d_tile_ptr, tile_ptr, "sho_plan_create: tile_ptr")) != SHO_OK ||
         (st = upload(&p->d_tile_ent, tile_ent, "sho_plan_create: tile_ent")) != SHO_OK ||
         (st = upload(&p->d_tile_list, tile_list, "sho_plan_create: tile_list")) != SHO_OK ||
-        (st = upload(&p->d_cainv, cainv, "sho_plan_create: cainv")) != SHO_OK) {
+        (st = upload(&p->d_cainv, cainv, "sho_plan_create: cainv")) != SHO_OK ||
+        (st = upload(&p->d_t2pos, t2pos, "sho_plan_create: t2pos")) != SHO_OK) {
         plan_free_device(p);
         delete p;
         return st;

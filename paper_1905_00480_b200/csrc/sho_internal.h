@@ -26,15 +26,22 @@ struct AtomDev {
     int32_t pad[2];
 };
 
-// one (atom image) that overlaps an add tile: unwrapped index i = j + m*N on each axis (32 bytes)
+// one (atom image) that overlaps an add tile: unwrapped index i = j + m*N on each axis.  Self-contained
+// (the atom's parameters are copied in) so that the add kernel fetches one 96-byte record per pair with
+// cp.async and never chases a pointer; 16-byte aligned
 struct AddEntry {
+    double pos[3];
+    double inv_sigma;    // 1 / sigma
+    double pref;         // (sqrt(pi) sigma)^(-1/2)
+    double wr, wi;       // conj(exp(2 pi i kfrac.m)): Bloch phase of the image, conjugated (reading A6)
     int32_t atom;
+    int32_t lo[3], hi[3];   // the atom's unwrapped inclusive box range
     int16_t m[3];
     uint8_t zmask;       // planes of the tile inside the box (bit k = plane k)
     int8_t ytlo, ythi;   // first / last 8-row block of the tile that the box touches
-    int8_t pad[3];
-    double wr, wi;       // conj(exp(2 pi i kfrac.m)): Bloch phase of the image, conjugated (reading A6)
+    uint8_t pad[3];
 };
+static_assert(sizeof(AddEntry) == 96, "AddEntry is fetched as six 16-byte cp.async pieces");
 
 // the (ny,nx) pairs with ny+nx <= numax, sorted by s = ny+nx (pair index s(s+1)/2 + nx), cut in MMA row
 // tiles of 8: tile mt needs nz <= numax - s_min(mt), i.e. nks[mt] K steps of 4, stored from block blk0[mt]
@@ -84,6 +91,8 @@ struct sho_plan {
     int32_t n_tile_list;
     sho::AddZTiles ztiles;
     uint16_t* d_cainv;                     // [nsho] coefficient n -> slot (block*32 + 4 q + t) of the z-stage A fragments
+    uint16_t* d_t2pos;                     // [256 + 8 nmt]: column of T2 that holds pair (ny,nx) (index 16 ny + nx; the zero
+                                           // column for ny+nx > numax), then the column of z-stage row 8 mt + q
     // workspace for the *_host calls
     void* ws_psi; size_t ws_psi_bytes;
     void* ws_c;   size_t ws_c_bytes;
