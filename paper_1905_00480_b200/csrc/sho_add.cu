@@ -27,13 +27,19 @@
 //           coefficients, times the conjugate Bloch phase of the image, into the A fragments of the z stage
 // so the latency-bound stages (E, C, T) of one warp overlap the tensor-core stages of the others.  All
 // three expansion stages run on DMMA.8x8x4.  Ring depths: x/y tables 3, everything else 2.
+#include <algorithm>
+#include <cstring>
+
 #include "sho_device.cuh"
 
 namespace sho {
 
+constexpr int kAddZTMax = 6;       // z-stage tasks one warp can own per step
+
+struct AddZTask { int32_t ca, fz, t2, w; };     // offsets inside a ring slot; w = nks | mt << 8 | pair << 16 (nks = 0: none)
+
 struct AddParams {
     GridDev g;
-    AddZTiles zt;
     const void* coeff;
     void* psi;
     const int32_t* tile_ptr;
@@ -46,22 +52,28 @@ struct AddParams {
     int32_t ntile0, ntile1;
     int32_t vec_ok;
     int32_t ng;                // pairs per pipeline step (NG)
-    int32_t npp;               // plane stride of T2 (doubles): 8 nmt + 2; column 8 nmt holds zeros
+    int32_t npp;               // columns per plane of T2: 8 nmt + 2; column 8 nmt holds zeros
+    int32_t nblk, nmt;         // K blocks of the z-stage A fragments per pair; row tiles of the z stage
+    int32_t zt;                // z-stage tasks per warp and step (<= kAddZTMax)
+    int32_t t_first;           // first thread that samples table points (the T stage runs on the last warps)
     long long band_stride;
+    double hz[SHO_NUMAX_MAX + 1];                  // sqrt(2^n / n!) for n <= numax, 0 beyond (padding functions vanish)
+    AddZTask ztask[kAddWarps][kAddZTMax];          // balanced against the T stage on the host (launch_t)
 };
 
 constexpr int kAddPoints = kAddTY + kAddTX + kAddTZ;    // 1D sample points per pair: 8 y blocks, 1 x block, 1 z block
 
-// shared-memory carve-up (doubles): [FXY: 3 NG x 9 KQ 32][FZ: 2 NG x KQ 32][CA: 2 NG x nblk P 32][T2: 2 NG x P 8 npp]
-// then [ENT: 2 NG records][META: 3 NG int32][ZPOS: 8 nmt uint16]
+// shared-memory carve-up (doubles): [FXY: 3 NG x 9 KQ 32][FZ: 2 NG x KQ 32][CA: 2 NG x nblk 32 P][T2: 2 NG x 8 npp P]
+// then [ENT: 2 NG records][META: 3 NG int32][ZPOS: 8 nmt uint16].  CA and T2 keep the real and imaginary
+// parts of complex data side by side, so one 16-byte access moves both.
 template <int KQ, int DT>
 struct AddSmem {
     static constexpr int P = Elem<DT>::cplx ? 2 : 1;
     static constexpr int FXYS = 9 * KQ * 32;
     static constexpr int FZS = KQ * 32;
     static constexpr int CPT = (KQ == 4) ? 4 : 2;            // coefficients a thread holds in flight per step
-    static __host__ __device__ int cas(int nblk) { return nblk * P * 32; }
-    static __host__ __device__ int t2s(int npp) { return P * kAddTZ * npp; }
+    static __host__ __device__ int cas(int nblk) { return nblk * 32 * P; }
+    static __host__ __device__ int t2s(int npp) { return kAddTZ * npp * P; }
     static __host__ __device__ size_t bytes(int ng, int nblk, int nmt)
     {
         const int npp = 8 * nmt + 2;
@@ -71,20 +83,25 @@ struct AddSmem {
     }
 };
 
-// phi_0..phi_{NV-1} as in sho_device.cuh::hermite_gauss, from the scalars of one atom
+// one real (P = 1) or one complex (P = 2) value as a single shared-memory access
+template <int P> struct PartVec;
+template <> struct PartVec<1> { double x; __device__ double re() const { return x; } __device__ double im() const { return 0.0; } };
+template <> struct __align__(16) PartVec<2> { double x, y; __device__ double re() const { return x; } __device__ double im() const { return y; } };
+
+// H_n(xi) exp(-xi^2/2) (sqrt(pi) sigma)^(-1/2) scale[n], n < NV, by the paper's monic recurrence (eq. (31),
+// PAPER.md:283-284) carried on p_n = H_n g; scale[n] = sqrt(2^n/n!) makes the functions orthonormal (reading A1)
 template <int NV>
-__device__ __forceinline__ void hermite_gauss_s(double u, double inv_sigma, double pref, const double* __restrict__ hnorm,
-                                                int numax, double (&out)[NV])
+__device__ __forceinline__ void hermite_gauss_s(double u, double inv_sigma, double pref, const double* __restrict__ scale,
+                                                double (&out)[NV])
 {
     const double xi = u * inv_sigma;
-    const double g = exp(-0.5 * xi * xi) * pref;
-    double hm = 0.0, hc = 1.0;
+    double pm = 0.0, pc = exp(-0.5 * xi * xi) * pref;
 #pragma unroll
     for (int n = 0; n < NV; ++n) {
-        out[n] = (n <= numax) ? hc * g * hnorm[n < SHO_NUMAX_MAX ? n : SHO_NUMAX_MAX] : 0.0;
-        const double hn = xi * hc - (0.5 * (double)n) * hm;
-        hm = hc;
-        hc = hn;
+        out[n] = pc * scale[n];
+        const double pn = xi * pc - (0.5 * (double)n) * pm;
+        pm = pc;
+        pc = pn;
     }
 }
 
@@ -120,13 +137,14 @@ __device__ __forceinline__ void ldg_pinned(const float* p, double& re)
 }
 
 template <int KQ, int DT>
-__global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddParams p)
+__global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const __grid_constant__ AddParams p)
 {
     using E = Elem<DT>;
     using real_t = typename E::real_t;
     using S = AddSmem<KQ, DT>;
     constexpr bool CPLX = E::cplx;
     constexpr int P = S::P;
+    using PV = PartVec<P>;
     constexpr int NV = 4 * KQ;                 // sampled functions per point (numax + 1 rounded up to 4)
     constexpr int NT = (KQ + 1) / 2;           // ny tiles of 8 in the x stage
     constexpr int NYT = kAddTY / 8;
@@ -137,12 +155,12 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
     extern __shared__ __align__(16) double smem[];
     const int nsho = p.g.nsho;
     const int NG = p.ng;
-    const int nblk = p.zt.nblk, nmt = p.zt.nmt, npp = p.npp;
-    const int CAS = S::cas(nblk), T2S = S::t2s(npp);
+    const int npp = p.npp;
+    const int CAS = S::cas(p.nblk), T2S = S::t2s(npp);    // doubles per pair
     double* FXY = smem;                                   // [3][NG][FXYS]  y blocks 0..7, x block 8
     double* FZ = FXY + (size_t)3 * NG * FXYS;             // [2][NG][FZS]
-    double* CA = FZ + (size_t)2 * NG * FZS;               // [2][NG][CAS]   A fragments of the z stage
-    double* T2 = CA + (size_t)2 * NG * CAS;               // [2][NG][T2S]
+    double* CA = FZ + (size_t)2 * NG * FZS;               // [2][NG][nblk][32][P]   A fragments of the z stage
+    double* T2 = CA + (size_t)2 * NG * CAS;               // [2][NG][8][npp][P]
     AddEntry* ENT = reinterpret_cast<AddEntry*>(T2 + (size_t)2 * NG * T2S);      // [2][NG]
     int32_t* META = reinterpret_cast<int32_t*>(ENT + 2 * NG);                    // [3][NG] zmask | ytlo << 8 | ythi << 16
     uint16_t* ZPOS = reinterpret_cast<uint16_t*>(META + 3 * NG);                 // [8 nmt] T2 column of z-stage row
@@ -155,7 +173,6 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
     const int tx = tile % p.ntile0, ty = (tile / p.ntile0) % p.ntile1, tz = tile / (p.ntile0 * p.ntile1);
     const int jx0 = tx * kAddTX, jy0 = ty * kAddTY, jz0 = tz * kAddTZ;
     const int Nx = p.g.ng[0], Ny = p.g.ng[1], Nz = p.g.ng[2];
-    const int numax = p.g.numax;
     const int ebeg = p.tile_ptr[tile], eend = p.tile_ptr[tile + 1];
     const int npairs = eend - ebeg;
     const int nG = (npairs + NG - 1) / NG;
@@ -174,7 +191,7 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
 
     // zero CA and T2 once: the padding entries of the z-stage A fragments and the zero column of T2 stay zero
     for (int i = tid; i < 2 * NG * (CAS + T2S); i += NTHR) CA[i] = 0.0;
-    for (int i = tid; i < 8 * nmt; i += NTHR) ZPOS[i] = p.t2pos[256 + i];
+    for (int i = tid; i < 8 * p.nmt; i += NTHR) ZPOS[i] = p.t2pos[256 + i];
 
     double D[NYT][P][2];
 #pragma unroll
@@ -190,23 +207,26 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
 #pragma unroll
         for (int ks = 0; ks < KQ; ++ks) t2off[nt][ks] = p.t2pos[16 * (8 * nt + 4 * (q & 1) + (q >> 1)) + 4 * ks + t];
 
-    // this thread's share of a group's coefficients: slot k = coefficient cn[k] of pair ci[k] -> CA offset co[k]
-    int ci[CPT], cn[CPT], co[CPT];
+    // this thread's share of a group's coefficients: slot k = coefficient cn[k] of pair ci[k] -> CA element co[k]
+    int ci[CPT], co[CPT];
+    const real_t* cptr[CPT];
+    const real_t* cbase = reinterpret_cast<const real_t*>(p.coeff) + (size_t)b * nsho * P;
 #pragma unroll
     for (int k = 0; k < CPT; ++k) {
         const int idx = tid + k * NTHR;
-        ci[k] = -1; cn[k] = 0; co[k] = 0;
+        ci[k] = -1; co[k] = 0; cptr[k] = cbase;
         if (idx < NG * nsho) {
             ci[k] = idx / nsho;
-            cn[k] = idx - ci[k] * nsho;
-            const int o = p.cainv[cn[k]];
-            co[k] = ci[k] * CAS + (o >> 5) * (32 * P) + (o & 31);
+            const int n = idx - ci[k] * nsho;
+            cptr[k] = cbase + (size_t)n * P;
+            co[k] = ci[k] * (CAS / P) + p.cainv[n];
         }
     }
-
-    const real_t* cbase = reinterpret_cast<const real_t*>(p.coeff) + (size_t)b * nsho * P;
     const size_t catom = (size_t)p.nbands * nsho * P;
     const bool cvec = p.vec_ok != 0;
+
+    // this thread's table points: point r of pair ti (T stage runs on the last warps, the z stage mostly on the first)
+    const int tpt = tid - p.t_first;
 
     cp_async_wait_all();
     __syncthreads();
@@ -225,7 +245,7 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
 #pragma unroll
                 for (int pp = 0; pp < P; ++pp) creg[k][pp] = 0.0;
                 if (ci[k] >= 0 && s * NG + ci[k] < npairs) {
-                    const real_t* c = cbase + (size_t)ENT[r2 * NG + ci[k]].atom * catom + (size_t)cn[k] * P;
+                    const real_t* c = cptr[k] + (size_t)ENT[r2 * NG + ci[k]].atom * catom;
                     if (CPLX) ldg_pinned(c, cvec, creg[k][0], creg[k][P - 1]);
                     else ldg_pinned(c, creg[k][0]);
                 }
@@ -233,12 +253,13 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
         }
         // ---------------- XY(s-2): every warp on its own plane ----------------
         if (s >= 2) {
-            for (int i = 0; i < NG; ++i) {
-                const int meta = META[r3m2 * NG + i];
+            const int32_t* meta_r = META + r3m2 * NG;
+            const double* fxy = FXY + (size_t)r3m2 * NG * FXYS + lane;
+            const PV* t2p = reinterpret_cast<const PV*>(T2 + (size_t)r2 * NG * T2S) + zl * npp;
+            for (int i = 0; i < NG; ++i, fxy += FXYS, t2p += kAddTZ * npp) {
+                const int meta = meta_r[i];
                 if (!((meta >> zl) & 1)) continue;
                 const int ytlo = (meta >> 8) & 0xff, ythi = (meta >> 16) & 0xff;
-                const double* fxy = FXY + (size_t)(r3m2 * NG + i) * FXYS + lane;
-                const double* t2p = T2 + (size_t)(r2 * NG + i) * T2S + (size_t)zl * npp;
 
                 double D1[NT][P][2];
 #pragma unroll
@@ -249,11 +270,11 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
                 for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
                     for (int ks = 0; ks < KQ; ++ks)
-                        if (8 * nt + 4 * ks <= numax) {                     // warp-uniform: the block holds some ny+nx <= numax
+                        if (8 * nt + 4 * ks <= 4 * KQ - 4) {               // the block holds some ny+nx <= numax (numax >= 4 KQ - 4)
                             const double a = fxy[(8 * KQ + ks) * 32];
-#pragma unroll
-                            for (int pp = 0; pp < P; ++pp)
-                                dmma(D1[nt][pp][0], D1[nt][pp][1], a, t2p[(size_t)pp * kAddTZ * npp + t2off[nt][ks]]);
+                            const PV bv = t2p[t2off[nt][ks]];
+                            dmma(D1[nt][0][0], D1[nt][0][1], a, bv.re());
+                            if (CPLX) dmma(D1[nt][P - 1][0], D1[nt][P - 1][1], a, bv.im());
                         }
 #pragma unroll
                 for (int yt = 0; yt < NYT; ++yt)
@@ -271,30 +292,37 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
         if (s >= 1 && s - 1 < nG) {
             const int r2m1 = r2 ^ 1;
             const int cnt = min(NG, npairs - (s - 1) * NG);
-            for (int task = zl; task < cnt * nmt; task += kAddWarps) {
-                const int i = task / nmt, mt = task - i * nmt;
-                const double* fz = FZ + (size_t)(r2m1 * NG + i) * FZS + lane;
-                const double* ap = CA + (size_t)(r2m1 * NG + i) * CAS + (size_t)p.zt.blk0[mt] * (32 * P) + lane;
-                const int nks = p.zt.nks[mt];
+            const double* fz_r = FZ + (size_t)r2m1 * NG * FZS + lane;
+            const PV* ca_r = reinterpret_cast<const PV*>(CA + (size_t)r2m1 * NG * CAS) + lane;
+            PV* t2_r = reinterpret_cast<PV*>(T2 + (size_t)r2m1 * NG * T2S) + 2 * t * npp;
+            for (int k = 0; k < p.zt; ++k) {
+                const AddZTask zd = p.ztask[zl][k];
+                const int nks = zd.w & 0xff, mt = (zd.w >> 8) & 0xff;
+                if (nks == 0 || (zd.w >> 16) >= cnt) continue;
+                const double* fz = fz_r + zd.fz;
+                const PV* ap = ca_r + zd.ca;
                 double d[P][2];
 #pragma unroll
                 for (int pp = 0; pp < P; ++pp) d[pp][0] = d[pp][1] = 0.0;
-                for (int ks = 0; ks < nks; ++ks) {
-                    const double bfr = fz[ks * 32];                            // B[k = nz][col = plane]
 #pragma unroll
-                    for (int pp = 0; pp < P; ++pp) dmma(d[pp][0], d[pp][1], ap[(ks * P + pp) * 32], bfr);
-                }
-                double* o = T2 + (size_t)(r2m1 * NG + i) * T2S + (size_t)(2 * t) * npp + ZPOS[8 * mt + q];
-#pragma unroll
-                for (int pp = 0; pp < P; ++pp) {
-                    o[(size_t)pp * kAddTZ * npp] = d[pp][0];
-                    o[(size_t)pp * kAddTZ * npp + npp] = d[pp][1];
-                }
+                for (int ks = 0; ks < KQ; ++ks)
+                    if (ks < nks) {
+                        const double bfr = fz[ks * 32];                          // B[k = nz][col = plane]
+                        const PV av = ap[ks * 32];
+                        dmma(d[0][0], d[0][1], av.re(), bfr);
+                        if (CPLX) dmma(d[P - 1][0], d[P - 1][1], av.im(), bfr);
+                    }
+                PV* o = t2_r + zd.t2 + ZPOS[8 * mt + q];
+                PV o0, o1;
+                o0.x = d[0][0]; o1.x = d[0][1];
+                if constexpr (CPLX) { o0.y = d[1][0]; o1.y = d[1][1]; }
+                o[0] = o0;
+                o[npp] = o1;
             }
         }
         // ---------------- T(s): 1D functions (step a1) in fragment order; scatter of C(s) ----------------
         if (s < nG) {
-            for (int it = tid; it < NG * kAddPoints; it += NTHR) {
+            for (int it = tpt; it >= 0 && it < NG * kAddPoints; it += NTHR) {
                 const int i = it / kAddPoints, r = it - i * kAddPoints;
                 if (s * NG + i >= npairs) break;
                 const AddEntry* en = ENT + r2 * NG + i;
@@ -305,7 +333,7 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
                 const bool valid = j < N && iu >= en->lo[d] && iu <= en->hi[d];
                 double v[NV];
                 if (valid) {
-                    hermite_gauss_s<NV>(displacement(iu, p.g.h, en->pos[d]), en->inv_sigma, en->pref, p.g.hnorm, numax, v);
+                    hermite_gauss_s<NV>(displacement(iu, p.g.h, en->pos[d]), en->inv_sigma, en->pref, p.hz, v);
                 } else {
 #pragma unroll
                     for (int n = 0; n < NV; ++n) v[n] = 0.0;
@@ -327,19 +355,21 @@ __global__ void __launch_bounds__(kAddWarps * 32, 2) sho_add_kernel(const AddPar
                                           ? ((int)en->zmask | ((int)en->ytlo << 8) | ((int)en->ythi << 16)) : 0;
             }
             // coefficients of the group: conjugate image phase, scatter into the z-stage A fragments
-            double* ca = CA + (size_t)r2 * NG * CAS;
+            PV* ca = reinterpret_cast<PV*>(CA + (size_t)r2 * NG * CAS);
 #pragma unroll
             for (int k = 0; k < CPT; ++k)
                 if (ci[k] >= 0 && s * NG + ci[k] < npairs) {
-                    if (!CPLX) {
-                        ca[co[k]] = creg[k][0];
+                    PV o;
+                    if constexpr (!CPLX) {
+                        o.x = creg[k][0];
                     } else {
                         const AddEntry* en = ENT + r2 * NG + ci[k];
                         const double wr = en->wr, wi = en->wi;
                         const double re = creg[k][0], im = creg[k][P - 1];
-                        ca[co[k]] = re * wr - im * wi;
-                        ca[co[k] + 32] = re * wi + im * wr;
+                        o.x = re * wr - im * wi;
+                        o.y = re * wi + im * wr;
                     }
+                    ca[co[k]] = o;
                 }
         }
         cp_async_wait_all();
@@ -391,9 +421,10 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
 {
     using S = AddSmem<KQ, DT>;
     constexpr bool CPLX = Elem<DT>::cplx;
+    constexpr int P = S::P;
     AddParams p;
+    std::memset(&p, 0, sizeof(p));
     p.g = pl->g;
-    p.zt = pl->ztiles;
     p.coeff = coeff; p.psi = psi;
     p.tile_ptr = pl->d_tile_ptr; p.tile_ent = pl->d_tile_ent; p.tile_list = pl->d_tile_list;
     p.cainv = pl->d_cainv; p.t2pos = pl->d_t2pos;
@@ -405,17 +436,50 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
     const size_t valign = CPLX ? esz : 2 * esz;
     p.vec_ok = ((reinterpret_cast<uintptr_t>(psi) % valign) == 0) && (CPLX || (pl->g.ng[0] % 2 == 0));
     if (CPLX && (reinterpret_cast<uintptr_t>(coeff) % esz) != 0) p.vec_ok = 0;
-    p.npp = 8 * pl->ztiles.nmt + 2;
+    const AddZTiles& zt = pl->ztiles;
+    p.nblk = zt.nblk; p.nmt = zt.nmt;
+    p.npp = 8 * zt.nmt + 2;
+    for (int n = 0; n <= SHO_NUMAX_MAX; ++n) p.hz[n] = (n <= pl->g.numax) ? pl->g.hnorm[n] : 0.0;
     // pairs per pipeline step: as many as fit two CTAs per SM and CPT coefficients per thread (at most 4)
     const size_t budget = 112 * 1024;
     int ng = 1;
-    while (ng < 4 && S::bytes(ng + 1, pl->ztiles.nblk, pl->ztiles.nmt) <= budget &&
+    while (ng < 4 && S::bytes(ng + 1, zt.nblk, zt.nmt) <= budget &&
            (ng + 1) * pl->g.nsho <= S::CPT * kAddWarps * 32) ++ng;
     p.ng = ng;
-    const size_t smem = S::bytes(ng, pl->ztiles.nblk, pl->ztiles.nmt);
+    const size_t smem = S::bytes(ng, zt.nblk, zt.nmt);
     if (smem > 227 * 1024 || pl->g.nsho > S::CPT * kAddWarps * 32) {
         set_error("sho_add: numax = %d needs %zu bytes of shared memory (> 227 KB)", pl->g.numax, smem);
         return SHO_ERR_UNSUPPORTED;
+    }
+    // The T stage (ng * 80 table points, one per thread) runs on the last warps; the z-stage tasks (pair, row
+    // tile) go to the least loaded warp, a table point batch counting as kTCost K steps of the z stage.
+    {
+        const int npts = ng * kAddPoints;
+        const int nthr = kAddWarps * 32;
+        p.t_first = std::max(0, nthr - ((npts + 31) / 32) * 32);
+        if (npts > nthr) p.t_first = 0;
+        const int kTCost = 10;
+        int load[kAddWarps], cnt[kAddWarps];
+        for (int w = 0; w < kAddWarps; ++w) {
+            const int lo = std::max(w * 32, p.t_first), hi = std::min((w + 1) * 32, p.t_first + npts);
+            load[w] = (hi > lo) ? kTCost * ((npts + nthr - 1) / nthr) : 0;
+            cnt[w] = 0;
+        }
+        for (int i = 0; i < ng; ++i)
+            for (int mt = 0; mt < zt.nmt; ++mt) {
+                int best = -1;
+                for (int w = 0; w < kAddWarps; ++w)
+                    if (cnt[w] < kAddZTMax && (best < 0 || load[w] < load[best])) best = w;
+                if (best < 0) { set_error("sho_add: z-stage task table overflow"); return SHO_ERR_UNSUPPORTED; }
+                AddZTask& zk = p.ztask[best][cnt[best]++];
+                zk.ca = i * (S::cas(zt.nblk) / P) + zt.blk0[mt] * 32;
+                zk.fz = i * S::FZS;
+                zk.t2 = i * (S::t2s(p.npp) / P);
+                zk.w = zt.nks[mt] | (mt << 8) | (i << 16);
+                load[best] += 1 + zt.nks[mt];
+            }
+        p.zt = 0;
+        for (int w = 0; w < kAddWarps; ++w) p.zt = std::max(p.zt, cnt[w]);
     }
     auto kern = sho_add_kernel<KQ, DT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
