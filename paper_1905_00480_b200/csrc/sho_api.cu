@@ -52,9 +52,9 @@ static sho_status upload(T** dst, const std::vector<T>& src, const char* what)
 static void plan_free_device(sho_plan* p)
 {
     cudaFree(p->d_atoms); cudaFree(p->d_order); cudaFree(p->d_nxyz);
-    cudaFree(p->d_tile_ptr); cudaFree(p->d_tile_ent); cudaFree(p->d_tile_list); cudaFree(p->d_cainv); cudaFree(p->d_t2pos);
+    cudaFree(p->d_tile_ptr); cudaFree(p->d_tile_ent); cudaFree(p->d_tile_list); cudaFree(p->d_cainv); cudaFree(p->d_t2pos); cudaFree(p->d_cidx);
     cudaFree(p->ws_psi); cudaFree(p->ws_c);
-    p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr;
+    p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr; p->d_cidx = nullptr;
     p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr;
     p->ws_psi = nullptr; p->ws_c = nullptr;
 }
@@ -122,7 +122,7 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
     sho_plan* p = new (std::nothrow) sho_plan();
     if (!p) { set_error("sho_plan_create: host allocation failed"); return SHO_ERR_OOM; }
     p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr;
-    p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr;
+    p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr; p->d_cidx = nullptr;
     p->ws_psi = nullptr; p->ws_c = nullptr; p->ws_psi_bytes = 0; p->ws_c_bytes = 0;
     p->rcut_sigma = rcut_sigma;
     p->dtype = dtype;
@@ -348,6 +348,10 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
             for (int nx = 0; nx <= s; ++nx) t2pos[(size_t)256 + s * (s + 1) / 2 + nx] = t2pos[(size_t)16 * (s - nx) + nx];
     }
 
+    // ---- inverse of cainv: the coefficient that lane 4 q + t holds in K block blk of the z-stage A fragments ----
+    std::vector<uint16_t> cidx((size_t)std::max(p->ztiles.nblk, 1) * 32, (uint16_t)0xffff);
+    for (int n = 0; n < g.nsho; ++n) cidx[cainv[(size_t)n]] = (uint16_t)n;
+
     // ---- device mirrors ----
     cudaError_t e = cudaGetDevice(&p->device);
     if (e != cudaSuccess) { sho_status s = cuda_fail(e, "sho_plan_create: cudaGetDevice (no CUDA device?)"); delete p; return s; }
@@ -359,7 +363,8 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
         (st = upload(&p->d_tile_ent, tile_ent, "sho_plan_create: tile_ent")) != SHO_OK ||
         (st = upload(&p->d_tile_list, tile_list, "sho_plan_create: tile_list")) != SHO_OK ||
         (st = upload(&p->d_cainv, cainv, "sho_plan_create: cainv")) != SHO_OK ||
-        (st = upload(&p->d_t2pos, t2pos, "sho_plan_create: t2pos")) != SHO_OK) {
+        (st = upload(&p->d_t2pos, t2pos, "sho_plan_create: t2pos")) != SHO_OK ||
+        (st = upload(&p->d_cidx, cidx, "sho_plan_create: cidx")) != SHO_OK) {
         plan_free_device(p);
         delete p;
         return st;

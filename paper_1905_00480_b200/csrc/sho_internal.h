@@ -91,6 +91,7 @@ struct sho_plan {
     int32_t n_tile_list;
     sho::AddZTiles ztiles;
     uint16_t* d_cainv;                     // [nsho] coefficient n -> slot (block*32 + 4 q + t) of the z-stage A fragments
+    uint16_t* d_cidx;                      // [nblk][32] inverse of cainv (0xffff: padding element)
     uint16_t* d_t2pos;                     // [256 + 8 nmt]: column of T2 that holds pair (ny,nx) (index 16 ny + nx; the zero
                                            // column for ny+nx > numax), then the column of z-stage row 8 mt + q
     // workspace for the *_host calls
