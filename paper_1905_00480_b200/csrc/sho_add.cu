@@ -58,18 +58,18 @@ struct AddParams {
 };
 
 // shared-memory carve-up (doubles): [FXY: RD x 9 KQ 32][T2: RD x 2 x 8 npp][FZ: npw x KQ 32][STG: npw x stg]
-// [ENT: npw x 2 records] then [META: RD int32][ZPOS: 8 nmt uint16][CIDX: 32 nblk uint16][mbarriers: full RD, empty RD]
+// [EXPT: 64][ENT: npw x 2 records] then [META: RD int32][ZPOS: 8 nmt uint16][CIDX: 32 nblk uint16][mbarriers: full RD, empty RD]
 template <int KQ>
 struct AddSmem {
     static constexpr int FXYS = 9 * KQ * 32;
     static constexpr int FZS = KQ * 32;
     static __host__ __device__ int t2s(int npp) { return 2 * kAddTZ * npp; }
-    // raw coefficients of one pair, both channels, as the kernel copies them from global memory
-    static __host__ __device__ int stg(int nsho, int real_bytes) { return ((2 * nsho * real_bytes + 15) / 16) * 2; }
-    static __host__ __device__ size_t bytes(int rd, int npw, int nmt, int nblk, int nsho, int real_bytes)
+    // z-stage A fragments of one pair in the element type of the data: [K block][lane][channel]
+    static __host__ __device__ int stg(int nblk, int real_bytes) { return ((64 * nblk * real_bytes + 15) / 16) * 2; }
+    static __host__ __device__ size_t bytes(int rd, int npw, int nmt, int nblk, int real_bytes)
     {
         const int npp = 8 * nmt + 2;
-        size_t b = 8 * ((size_t)rd * (FXYS + t2s(npp)) + (size_t)npw * (FZS + stg(nsho, real_bytes)));
+        size_t b = 8 * ((size_t)rd * (FXYS + t2s(npp)) + (size_t)npw * (FZS + stg(nblk, real_bytes)) + 64);
         b += (size_t)npw * 2 * sizeof(AddEntry);
         b += (size_t)rd * 4 + (size_t)8 * nmt * 2 + (size_t)32 * nblk * 2;
         b = (b + 7) & ~(size_t)7;
@@ -77,14 +77,39 @@ struct AddSmem {
     }
 };
 
+// exp(x), x <= 0, in 11 FP64-pipe instructions (the library routine takes about 28; the producer warps share the
+// FP64 pipe with the DMMAs of the XY warps, so every instruction there waits its turn):
+//   x = (64 k + j) ln2/64 + r,  |r| <= ln2/128,   exp(x) = 2^k 2^(j/64) exp(r),
+// 2^(j/64) from a 64-entry table in shared memory, exp(r) by its Taylor polynomial of degree 5 (remainder
+// r^6/720 < 4e-17), 2^k by an integer add on the exponent field.  Relative error <= 4e-16 (checked against 60-digit
+// arithmetic on 2e5 arguments in [-700, 0]).
+__device__ __forceinline__ double exp_neg(double x, const double* __restrict__ tab)
+{
+    x = fmax(x, -700.0);
+    const double magic = 6755399441055744.0;                                   // 1.5 * 2^52: rounds to an integer in the low word
+    const double tn = fma(x, 92.33248261689366, magic);                    // 64 / ln2
+    const int n = __double2loint(tn);
+    const double fn = tn - magic;
+    double r = fma(fn, -0.010830424695996044, x);                              // ln2/64, high 34 bits (0x1.62e42fef8p-7): exact product
+    r = fma(fn, -2.5310172166650877e-13, r);                                   // ln2/64, the rest
+    double q = fma(r, 8.3333333333333332e-3, 4.1666666666666664e-2);
+    q = fma(q, r, 1.6666666666666666e-1);
+    q = fma(q, r, 0.5);
+    q = fma(q, r, 1.0);
+    q = fma(q, r, 1.0);
+    const double tj = tab[n & 63];
+    const int hi = __double2hiint(tj) + ((n >> 6) << 20);
+    return q * __hiloint2double(hi, __double2loint(tj));
+}
+
 // H_n(xi) exp(-xi^2/2) (sqrt(pi) sigma)^(-1/2) scale[n], n < NV, by the paper's monic recurrence (eq. (31),
 // PAPER.md:283-284) carried on p_n = H_n g; scale[n] = sqrt(2^n/n!) makes the functions orthonormal (reading A1)
 template <int NV>
 __device__ __forceinline__ void hermite_gauss_s(double u, double inv_sigma, double pref, const double* __restrict__ scale,
-                                                double (&out)[NV])
+                                                const double* __restrict__ exptab, double (&out)[NV])
 {
     const double xi = u * inv_sigma;
-    double pm = 0.0, pc = exp(-0.5 * xi * xi) * pref;
+    double pm = 0.0, pc = exp_neg(-0.5 * xi * xi, exptab) * pref;
 #pragma unroll
     for (int n = 0; n < NV; ++n) {
         out[n] = pc * scale[n];
@@ -115,13 +140,15 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, int parity)
     }
 }
 
-// asynchronous global -> shared copy of 4, 8 or 16 bytes (both addresses aligned to the size)
-__device__ __forceinline__ void cp_async(void* smem_dst, const void* gmem_src, int bytes)
+// asynchronous global -> shared copy of 4, 8 or 16 bytes (both addresses aligned to the size); with
+// take == false nothing is read and the destination is filled with zeros
+__device__ __forceinline__ void cp_async(void* smem_dst, const void* gmem_src, int bytes, bool take = true)
 {
     const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
-    if (bytes == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src) : "memory");
-    else if (bytes == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(gmem_src) : "memory");
-    else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(d), "l"(gmem_src) : "memory");
+    const int n = take ? bytes : 0;
+    if (bytes == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(d), "l"(gmem_src), "r"(n) : "memory");
+    else if (bytes == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(d), "l"(gmem_src), "r"(n) : "memory");
+    else asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;\n" ::"r"(d), "l"(gmem_src), "r"(n) : "memory");
 }
 
 template <int KQ, int DT>
@@ -148,10 +175,11 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
     double* FXY = smem;                                   // [RD][9 KQ][32]     y blocks 0..7, x block 8
     double* T2 = FXY + (size_t)RD * FXYS;                 // [RD][2][8][npp]
     const int NPW = p.npw;
-    const int STGS = S::stg(nsho, (int)sizeof(real_t));
+    const int STGS = S::stg(p.nblk, (int)sizeof(real_t));
     double* FZ = T2 + (size_t)RD * T2S;                   // [npw][KQ][32]
-    double* STG = FZ + (size_t)NPW * FZS;                 // [npw][STGS]   raw coefficients of the pair in production
-    AddEntry* ENTW = reinterpret_cast<AddEntry*>(STG + (size_t)NPW * STGS);      // [npw][2]  this and the next record
+    double* STG = FZ + (size_t)NPW * FZS;                 // [npw][STGS]   z-stage A fragments of the pair in production, element type of the data
+    double* EXPT = STG + (size_t)NPW * STGS;              // [64]  2^(j/64), see exp_neg
+    AddEntry* ENTW = reinterpret_cast<AddEntry*>(EXPT + 64);                     // [npw][2]  this and the next record
     int32_t* META = reinterpret_cast<int32_t*>(ENTW + 2 * NPW);                  // [RD] zmask | ytlo << 8 | ythi << 16
     uint16_t* ZPOS = reinterpret_cast<uint16_t*>(META + RD);                     // [8 nmt] T2 column of z-stage row
     uint16_t* CIDX = ZPOS + 8 * nmt;                                             // [nblk][32] coefficient of an A-fragment element
@@ -175,6 +203,7 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
     for (int i = tid; i < RD * T2S; i += kAddThreads) T2[i] = 0.0;
     for (int i = tid; i < 8 * nmt; i += kAddThreads) ZPOS[i] = p.t2pos[256 + i];
     for (int i = tid; i < 32 * p.nblk; i += kAddThreads) CIDX[i] = p.cidx[i];
+    if (tid < 64) EXPT[tid] = exp2((double)tid * (1.0 / 64.0));
     if (tid == 0) {
         for (int i = 0; i < RD; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, kAddXYWarps); }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
@@ -328,7 +357,6 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
         const bool two = CPLX || (b0 + 1 < p.nbands);      // second channel exists
         // copy granule: one complex coefficient when its alignment is known, else one real number
         const int gran = (CPLX && p.vec_ok) ? 2 : 1;       // reals per cp.async
-        const int ncopy = (CPLX ? 2 * nsho : (two ? 2 * nsho : nsho)) / gran;
         auto fetch_entry = [&](int g, int buf) {
             if (lane < 6 && g < npairs)
                 cp_async(reinterpret_cast<char*>(entw + buf) + 16 * lane,
@@ -340,12 +368,20 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
         int slot = pw % RD, k = pw / RD, ebuf = 0;
         for (int g = pw; g < npairs; g += NPW, ebuf ^= 1) {
             const AddEntry* en = entw + ebuf;
-            // ---- coefficients of the pair -> staging (complex: [n][re, im]; two real bands: [band][n]) ----
+            // ---- coefficients of the pair -> A fragments of the z stage.  Every coefficient sits in exactly one
+            // fragment element: the lane copies its own (cp.async gather, zero fill for the padding elements) ----
             {
                 const real_t* c = cbase + (size_t)en->atom * catom;
-                for (int i = lane; i < ncopy; i += 32) {
-                    // two real bands are nsho apart in c and in the staging buffer alike
-                    cp_async(stg + (size_t)i * gran, c + (size_t)i * gran, (int)sizeof(real_t) * gran);
+                for (int blk = 0; blk < p.nblk; ++blk) {
+                    const int n = CIDX[blk * 32 + lane];
+                    const bool has = n != 0xffff;
+                    const real_t* src = c + (has ? (size_t)n * P : 0);
+                    real_t* dst = stg + (size_t)(blk * 32 + lane) * 2;
+                    if (CPLX && gran == 2) cp_async(dst, src, 2 * (int)sizeof(real_t), has);
+                    else {
+                        cp_async(dst, src, (int)sizeof(real_t), has);
+                        cp_async(dst + 1, src + (CPLX ? 1 : nsho), (int)sizeof(real_t), has && two);
+                    }
                 }
             }
             fetch_entry(g + NPW, ebuf ^ 1);
@@ -353,48 +389,27 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
             const int ytlo = en->ytlo, ythi = en->ythi;
             if (k >= 1) mbar_wait(empty + slot, (k - 1) & 1);        // the slot's previous pair has been consumed
             double* fxy_s = FXY + (size_t)slot * FXYS;
-            // ---- 1D functions (step a1) in fragment order: block (y: 0..7, x: 8), point r & 7 holds element
-            // [k = n & 3] of K step n >> 2.  First the z points (lanes 0..7) and x points (lanes 8..15) ----
+            // ---- 1D functions (step a1) in fragment order: block (y: 0..7, x: 8; z: this warp's own buffer), point
+            // r & 7 holds element [k = n & 3] of K step n >> 2.  Points of the pair: 8 z planes, 8 x columns, then
+            // the rows of the 8-row blocks the box touches (the others are never read); 32 points per pass ----
             {
-                const int d = lane < 8 ? 2 : 0;
-                const int j = (d == 2 ? jz0 : jx0) + (lane & 7);
-                const int N = p.g.ng[d];
-                const int iu = j + (int)en->m[d] * N;
-                const bool valid = lane < 16 && j < N && iu >= en->lo[d] && iu <= en->hi[d];
-                double v[NV];
-                if (valid) {
-                    hermite_gauss_s<NV>(displacement(iu, p.g.h, en->pos[d]), inv_sigma, pref, p.hz, v);
-                } else {
-#pragma unroll
-                    for (int n = 0; n < NV; ++n) v[n] = 0.0;
-                }
-                if (lane < 16) {
-                    double* dst = (d == 2 ? fzw : fxy_s + 8 * KQ * 32) + (lane & 7) * 4;
-#pragma unroll
-                    for (int kk = 0; kk < KQ; ++kk) {
-                        double2 a, c;
-                        a.x = v[4 * kk]; a.y = v[4 * kk + 1]; c.x = v[4 * kk + 2]; c.y = v[4 * kk + 3];
-                        *reinterpret_cast<double2*>(dst + kk * 32) = a;
-                        *reinterpret_cast<double2*>(dst + kk * 32 + 2) = c;
-                    }
-                }
-            }
-            // ---- the y points of the 8-row blocks the box touches, 32 rows per pass ----
-            {
-                const double posy = en->pos[1];
-                const int my = (int)en->m[1] * Ny, loy = en->lo[1], hiy = en->hi[1];
-                for (int r = 8 * ytlo + lane; r < 8 * ythi + 8; r += 32) {
-                    const int j = jy0 + r;
-                    const int iu = j + my;
-                    const bool valid = j < Ny && iu >= loy && iu <= hiy;
+                const int npts = 16 + 8 * (ythi - ytlo + 1);
+                for (int i = lane; i < npts; i += 32) {
+                    const int d = i < 8 ? 2 : (i < 16 ? 0 : 1);
+                    const int r = (d == 1) ? 8 * ytlo + i - 16 : (i & 7);            // row of the tile / point of the block
+                    const int j = (d == 1 ? jy0 : (d == 2 ? jz0 : jx0)) + r;
+                    const int N = p.g.ng[d];
+                    const int iu = j + (int)en->m[d] * N;
+                    const bool valid = j < N && iu >= en->lo[d] && iu <= en->hi[d];
                     double v[NV];
                     if (valid) {
-                        hermite_gauss_s<NV>(displacement(iu, p.g.h, posy), inv_sigma, pref, p.hz, v);
+                        hermite_gauss_s<NV>(displacement(iu, p.g.h, en->pos[d]), inv_sigma, pref, p.hz, EXPT, v);
                     } else {
 #pragma unroll
                         for (int n = 0; n < NV; ++n) v[n] = 0.0;
                     }
-                    double* dst = fxy_s + ((r >> 3) * KQ) * 32 + (r & 7) * 4;
+                    double* dst = (d == 2) ? fzw + r * 4
+                                           : fxy_s + ((d == 0 ? 8 : (r >> 3)) * KQ) * 32 + (r & 7) * 4;
 #pragma unroll
                     for (int kk = 0; kk < KQ; ++kk) {
                         double2 a, c;
@@ -407,13 +422,13 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
             if (lane == 0) META[slot] = (int)en->zmask | (ytlo << 8) | (ythi << 16);
             asm volatile("cp.async.wait_all;\n" ::: "memory");
             __syncwarp();
-            // ---- z stage: T2[z][(ny,nx)] for the 8 planes.  Every coefficient sits in exactly one A-fragment
-            // element: the lane fetches its own from the staging buffer; two row tiles in flight ----
+            // ---- z stage: T2[z][(ny,nx)] for the 8 planes; two row tiles in flight ----
             {
                 double bz[KQ];
 #pragma unroll
                 for (int ks = 0; ks < KQ; ++ks) bz[ks] = fzw[ks * 32 + lane];       // B[k = nz][col = plane]
                 const double wr = en->wr, wi = en->wi;
+                const bool phased = !(wr == 1.0 && wi == 0.0);                  // warp-uniform; most images have none
                 double* t2 = T2 + (size_t)slot * T2S + (size_t)(2 * t) * npp;
                 for (int mt0 = 0; mt0 < nmt; mt0 += 2) {
                     double d[2][2][2];
@@ -428,13 +443,10 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
 #pragma unroll
                         for (int u = 0; u < 2; ++u)
                             if (ks < nks[u]) {                                    // warp-uniform
-                                const int n = CIDX[(p.zt.blk0[mt0 + u] + ks) * 32 + lane];
-                                double a0 = 0.0, a1 = 0.0;
-                                if (n != 0xffff) {
-                                    if (CPLX) { a0 = (double)stg[2 * n]; a1 = (double)stg[2 * n + 1]; }
-                                    else { a0 = (double)stg[n]; a1 = two ? (double)stg[nsho + n] : 0.0; }
-                                }
-                                if (CPLX) {                                       // conjugate Bloch phase of the image
+                                const real_t* ap = stg + (size_t)((p.zt.blk0[mt0 + u] + ks) * 32 + lane) * 2;
+                                double a0, a1;
+                                load2_rw(ap, a0, a1);
+                                if (CPLX && phased) {                             // conjugate Bloch phase of the image
                                     const double re = a0, im = a1;
                                     a0 = re * wr - im * wi;
                                     a1 = re * wi + im * wr;
@@ -489,15 +501,15 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
     const int rb = (int)(esz / (CPLX ? 2 : 1));
     const size_t budget = 224 * 1024;
     int npw = kAddPWarps;
-    while (npw > 1 && S::bytes(npw + 2, npw, zt.nmt, zt.nblk, pl->g.nsho, rb) > budget) --npw;
+    while (npw > 1 && S::bytes(npw + 2, npw, zt.nmt, zt.nblk, rb) > budget) --npw;
     int rd = npw + 2;
-    while (rd < 2 * npw + 2 && S::bytes(rd + 1, npw, zt.nmt, zt.nblk, pl->g.nsho, rb) <= budget) ++rd;
+    while (rd < 2 * npw + 2 && S::bytes(rd + 1, npw, zt.nmt, zt.nblk, rb) <= budget) ++rd;
     p.npw = npw; p.rd = rd;
     if (CPLX && (size_t)rd * (S::FXYS + S::t2s(p.npp)) < (size_t)kAddTZ * kAddTY * kAddTX) {
         set_error("sho_add: ring too small for the complex write-back exchange");
         return SHO_ERR_UNSUPPORTED;
     }
-    const size_t smem = S::bytes(rd, npw, zt.nmt, zt.nblk, pl->g.nsho, rb);
+    const size_t smem = S::bytes(rd, npw, zt.nmt, zt.nblk, rb);
     if (smem > 227 * 1024) {
         set_error("sho_add: numax = %d needs %zu bytes of shared memory (> 227 KB)", pl->g.numax, smem);
         return SHO_ERR_UNSUPPORTED;
