@@ -144,32 +144,42 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
     // x: steps of CWX columns (one 128-byte line per row) starting at a line-aligned column
     const int xs0 = floordiv(at.lo[0], CWX) * CWX;
     const int KX = (at.hi[0] - xs0 + CWX) / CWX;
-    const int KXG = (KX + G - 1) / G;
     // y: blocks of 8 rows (the N extent of the x-stage MMA)
     const int NYB = (nyl + 7) >> 3;
-    // complex data with an x-wrap: the accumulators are rotated once, at the first step that holds a column
-    // of the second image; the phase of the last image is folded into wz
+    // complex data with an x-wrap: the accumulators are rotated by exp(-2 pi i kfrac_x) once, before the first
+    // step of the second image; the phase of the last image is folded into wz.  If the image boundary falls
+    // inside a step, that step is scheduled twice with complementary column masks in its tables, so the inner
+    // loop never looks at single columns.  Schedule: KS steps, step k reads the columns of source step
+    // k - (k > kdup); the rotation happens before step krot.
     const bool xphase = CPLX && p.g.has_phase && p.g.periodic[0] && p.g.kfrac[0] != 0.0;
     const bool yphase = CPLX && p.g.has_phase && p.g.periodic[1] && p.g.kfrac[1] != 0.0;
-    int xB = INT_MAX, kx_rot = -1;
+    int xB = INT_MAX, krot = -1, kdup = INT_MAX;
     if (xphase) {
         const int mlo = floordiv(at.lo[0], Nx);
-        if (floordiv(at.hi[0], Nx) != mlo) { xB = (mlo + 1) * Nx; kx_rot = (xB - xs0) / CWX; }
+        if (floordiv(at.hi[0], Nx) != mlo) {
+            xB = (mlo + 1) * Nx;
+            krot = (xB - xs0) / CWX;
+            if ((xB - xs0) % CWX != 0) { kdup = krot; krot += 1; }
+        }
     }
+    const int KS = KX + (kdup != INT_MAX ? 1 : 0);
+    const int KXG = (KS + G - 1) / G;
 
     // ---------------- a1: sample the 1D tables on the fly, in fragment layout ----------------
-    const int nx_items = KX * CWX, ny_items = NYB * 8;
+    const int nx_items = KS * CWX, ny_items = NYB * 8;
     for (int it = tid; it < nx_items + ny_items + nzl; it += blockDim.x) {
         double v[NV];
         if (it < nx_items) {
-            const int j = it;
-            const int ix = xs0 + j;
-            const bool valid = ix >= at.lo[0] && ix <= at.hi[0];
+            const int k = it / CWX, r = it % CWX, tt = r / EPL, e = r % EPL;      // column r of the step = EPL * t + e
+            const int ix = xs0 + CWX * (k - (k > kdup ? 1 : 0)) + r;
+            const bool valid = ix >= at.lo[0] && ix <= at.hi[0] &&
+                               (kdup == INT_MAX || (k < krot ? ix < xB : ix >= xB));
             hermite_gauss<NV>(displacement(ix, p.g.h, at.pos[0]), at, p.g.hnorm, numax, valid, v);
-            const int kx = j / CWX, r = j % CWX, tt = r / EPL, e = r % EPL;      // column r of the step = EPL * t + e
+            // A fragments [step][mt][e / 2][lane = 4 nx + t][e & 1]: 16-byte loads, lanes 16 bytes apart (no bank conflicts)
 #pragma unroll
-            for (int n = 0; n < MP; ++n) fx[(((size_t)kx * EPL + e) * MT + (n >> 3)) * 32 + (n & 7) * 4 + tt] = v[n];
-            if (R) { fxr[2 * j] = v[MP]; fxr[2 * j + 1] = v[MP + R - 1]; }
+            for (int n = 0; n < MP; ++n)
+                fx[((((size_t)k * MT + (n >> 3)) * (EPL / 2) + (e >> 1)) * 32 + (n & 7) * 4 + tt) * 2 + (e & 1)] = v[n];
+            if (R) { fxr[2 * it] = v[MP]; fxr[2 * it + 1] = v[MP + R - 1]; }
         } else if (it < nx_items + ny_items) {
             const int pr = it - nx_items;                        // padded row slot
             int iy = at.lo[1] + pr;
@@ -207,12 +217,12 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
             }
         }
     }
-    // lane-span offsets of every x step (the steps that pad the last group repeat the last real step)
+    // lane-span offsets of every scheduled step (the steps that pad the last group repeat the last real step)
     for (int it = tid; it < KXG * G * 4; it += blockDim.x) {
-        const int kx = it >> 2, tt = it & 3;
-        const int x0 = xs0 + CWX * min(kx, KX - 1) + EPL * tt;
+        const int k = min(it >> 2, KS - 1), tt = it & 3;
+        const int x0 = xs0 + CWX * (k - (k > kdup ? 1 : 0)) + EPL * tt;
         const int off = p.g.periodic[0] ? x0 - floordiv(x0, Nx) * Nx : min(max(x0, 0), max(Nx - EPL, 0));
-        coloff[((kx / G) * 4 + tt) * G + (kx % G)] = off;
+        coloff[(((it >> 2) / G) * 4 + tt) * G + ((it >> 2) % G)] = off;
     }
     if (CPLX && tid == 0) {
         double sn, cs;
@@ -261,7 +271,8 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
             // unaligned psi or Nx not a multiple of the lane span: element-wise loads, every column wrapped
 #pragma unroll
             for (int j = 0; j < G; ++j) {
-                const int x0 = xs0 + CWX * min(kg * G + j, KX - 1) + EPL * t;
+                const int ks_ = min(kg * G + j, KS - 1);
+                const int x0 = xs0 + CWX * (ks_ - (ks_ > kdup ? 1 : 0)) + EPL * t;
 #pragma unroll
                 for (int e = 0; e < EPL; ++e) {
                     const int ix = x0 + e;
@@ -316,16 +327,16 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
                 for (int mt = 0; mt < MT; ++mt) C1[mt][0][0] = C1[mt][0][1] = C1[mt][1][0] = C1[mt][1][1] = 0.0;
                 ar[0][0] = ar[0][1] = ar[1][0] = ar[1][1] = 0.0;
 
-                for (int kg = 0; kg < KXG; ++kg) {
-                    const bool last = (kg == KXG - 1);
-                    real_t nxt[G][RAW];
-                    load_group(nxt, last ? nrp : rp, last ? 0 : kg + 1);
+                // this lane's table pointers, advanced by a constant per step (no address arithmetic in the loop)
+                const double* fxp = fx + (size_t)lane * 2;
+                const double* fxrp = fxr + (size_t)t * EPL * 2;
+                auto compute_group = [&](const real_t (&buf)[G][RAW], int kg) {
 #pragma unroll
                     for (int j = 0; j < G; ++j) {
-                        const int kx = kg * G + j;
-                        if (kx < KX) {
-                            const bool rot = CPLX && kx == kx_rot;
-                            if (rot) {
+                        const int k = kg * G + j;
+                        if (k < KS) {
+                            if (CPLX && k == krot) {
+                                // the columns so far belong to the previous x image: rotate what they have summed
                                 const double cr = phx[0], ci = phx[1];
 #pragma unroll
                                 for (int mt = 0; mt < MT; ++mt)
@@ -345,30 +356,30 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
                                 }
                             }
                             // ---- a3: x contraction, EPL K steps of 4 columns ----
+                            double afr[MT][EPL];
+#pragma unroll
+                            for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+                                for (int eh = 0; eh < EPL / 2; ++eh) {
+                                    const double2 a2 = *reinterpret_cast<const double2*>(fxp + (mt * (EPL / 2) + eh) * 64);
+                                    afr[mt][2 * eh] = a2.x; afr[mt][2 * eh + 1] = a2.y;
+                                }
 #pragma unroll
                             for (int e = 0; e < EPL; ++e) {
                                 double ve[P];
 #pragma unroll
-                                for (int pp = 0; pp < P; ++pp) ve[pp] = (double)cur[j][e * P + pp];
-                                if (rot && xs0 + CWX * kx + EPL * t + e < xB) {
-                                    // column of the first image inside the rotation step: same rotation for the value
-                                    const double cr = phx[0], ci = phx[1];
-                                    const double re = ve[0], im = ve[P - 1];
-                                    ve[0] = re * cr - im * ci;
-                                    ve[P - 1] = re * ci + im * cr;
-                                }
+                                for (int pp = 0; pp < P; ++pp) ve[pp] = (double)buf[j][e * P + pp];
 #pragma unroll
                                 for (int mt = 0; mt < MT; ++mt) {
-                                    const double afr = fx[(((size_t)kx * EPL + e) * MT + mt) * 32 + lane];
                                     if (CPLX) {
-                                        dmma(C1[mt][0][0], C1[mt][0][1], afr, ve[0]);
-                                        dmma(C1[mt][1][0], C1[mt][1][1], afr, ve[P - 1]);
+                                        dmma(C1[mt][0][0], C1[mt][0][1], afr[mt][e], ve[0]);
+                                        dmma(C1[mt][1][0], C1[mt][1][1], afr[mt][e], ve[P - 1]);
                                     } else {
-                                        dmma(C1[mt][e & 1][0], C1[mt][e & 1][1], afr, ve[0]);
+                                        dmma(C1[mt][e & 1][0], C1[mt][e & 1][1], afr[mt][e], ve[0]);
                                     }
                                 }
                                 if (R) {
-                                    const double2 f = *reinterpret_cast<const double2*>(&fxr[2 * (kx * CWX + EPL * t + e)]);
+                                    const double2 f = *reinterpret_cast<const double2*>(fxrp + 2 * e);
 #pragma unroll
                                     for (int pp = 0; pp < P; ++pp) {
                                         ar[0][pp] = fma(f.x, ve[pp], ar[0][pp]);
@@ -376,12 +387,26 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
                                     }
                                 }
                             }
+                            fxp += MT * 32 * EPL;
+                            fxrp += CWX * 2;
                         }
                     }
+                };
+                // two register buffers take turns (no copies); only a row block with an odd number of groups ends
+                // with the next block's first group in the wrong one
+                real_t nxt[G][RAW];
+                for (int kg = 0; kg < KXG; kg += 2) {
+                    load_group(nxt, (kg == KXG - 1) ? nrp : rp, (kg == KXG - 1) ? 0 : kg + 1);
+                    compute_group(cur, kg);
+                    if (kg + 1 < KXG) {
+                        load_group(cur, (kg + 1 == KXG - 1) ? nrp : rp, (kg + 1 == KXG - 1) ? 0 : kg + 2);
+                        compute_group(nxt, kg + 1);
+                    } else {
 #pragma unroll
-                    for (int j = 0; j < G; ++j)
+                        for (int j = 0; j < G; ++j)
 #pragma unroll
-                        for (int i = 0; i < RAW; ++i) cur[j][i] = nxt[j][i];
+                            for (int i = 0; i < RAW; ++i) cur[j][i] = nxt[j][i];
+                    }
                 }
 
                 // real data: the even / odd column chains meet
@@ -537,7 +562,7 @@ static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void
     p.atoms = pl->d_atoms; p.order = pl->d_order; p.nxyz = pl->d_nxyz;
     p.nbands = nbands;
     p.n_work_atoms = pl->n_nonempty;
-    p.kx_cap = (pl->max_n[0] + 2 * (CWX - 1)) / CWX + 1;
+    p.kx_cap = (pl->max_n[0] + 2 * (CWX - 1)) / CWX + 2;     // + the twice-scheduled image-boundary step
     p.yb_cap = (pl->max_n[1] + 7) / 8 + 1;
     p.nz_cap = pl->max_n[2] + 1;
     p.band_stride = (long long)pl->g.ng[0] * pl->g.ng[1] * pl->g.ng[2];
