@@ -367,6 +367,8 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
         __syncwarp();
         int slot = pw % RD, k = pw / RD, ebuf = 0;
         for (int g = pw; g < npairs; g += NPW, ebuf ^= 1) {
+            asm volatile("cp.async.wait_all;\n" ::: "memory");           // this pair's record (issued one iteration ago)
+            __syncwarp();
             const AddEntry* en = entw + ebuf;
             // ---- coefficients of the pair -> A fragments of the z stage.  Every coefficient sits in exactly one
             // fragment element: the lane copies its own (cp.async gather, zero fill for the padding elements) ----
@@ -384,7 +386,9 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
                     }
                 }
             }
-            fetch_entry(g + NPW, ebuf ^ 1);
+            asm volatile("cp.async.commit_group;\n" ::: "memory");
+            fetch_entry(g + NPW, ebuf ^ 1);                          // not waited for before the next iteration
+            asm volatile("cp.async.commit_group;\n" ::: "memory");
             const double inv_sigma = en->inv_sigma, pref = en->pref;
             const int ytlo = en->ytlo, ythi = en->ythi;
             if (k >= 1) mbar_wait(empty + slot, (k - 1) & 1);        // the slot's previous pair has been consumed
@@ -420,7 +424,7 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
                 }
             }
             if (lane == 0) META[slot] = (int)en->zmask | (ytlo << 8) | (ythi << 16);
-            asm volatile("cp.async.wait_all;\n" ::: "memory");
+            asm volatile("cp.async.wait_group 1;\n" ::: "memory");     // the coefficients; the next record may still fly
             __syncwarp();
             // ---- z stage: T2[z][(ny,nx)] for the 8 planes; two row tiles in flight ----
             {
