@@ -71,11 +71,11 @@ struct ProjSmem {
     static __host__ __device__ size_t wy(int yb) { return Elem<DT>::cplx ? (size_t)yb * 8 * 2 : 0; }
     static __host__ __device__ size_t fz(int nz) { return (size_t)nz * NV + (((size_t)nz * NV) & 1); }
     static __host__ __device__ size_t wz(int nz) { return Elem<DT>::cplx ? (size_t)nz * 2 : 0; }
-    static __host__ __device__ size_t t2() { return (size_t)2 * kProjWarps * P * TS; }
+    static __host__ __device__ size_t t2() { return (size_t)4 * kProjWarps * P * TS; }
     static __host__ __device__ size_t ints(int kx, int yb) { return (size_t)yb * 8 + (size_t)(kx + kProjG) * 4 + 4; }
     static __host__ __device__ size_t total_bytes(int kx, int yb, int nz)
     {
-        return 8 * (fx(kx) + fxr(kx) + fy(yb) + fys(yb) + wy(yb) + fz(nz) + wz(nz) + t2() + 2) + 4 * ints(kx, yb) + 16;
+        return 8 * (fx(kx) + fxr(kx) + fy(yb) + fys(yb) + wy(yb) + fz(nz) + wz(nz) + t2() + 2 + 4) + 4 * ints(kx, yb) + 16;
     }
 };
 
@@ -126,7 +126,8 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
     double* wz = fz + S::fz(p.nz_cap);                                // complex only: [z][2]
     double* t2s = wz + S::wz(p.nz_cap);                               // [2][W][P][TS]
     double* phx = t2s + S::t2();                                      // x rotation exp(-2 pi i kfrac_x) [re,im]
-    int32_t* rowoff = reinterpret_cast<int32_t*>(phx + 2);            // [padded row] element offset of the row
+    uint64_t* t2bar = reinterpret_cast<uint64_t*>(phx + 2);           // [4] one mbarrier per T2 buffer: its 8 planes are written
+    int32_t* rowoff = reinterpret_cast<int32_t*>(phx + 2 + 4);            // [padded row] element offset of the row
     int32_t* coloff = rowoff + (size_t)p.yb_cap * 8;                  // [group][t][step in group] element offset of the lane span
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -229,6 +230,10 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
         sincospi(-2.0 * p.g.kfrac[0], &sn, &cs);
         phx[0] = cs; phx[1] = sn;
     }
+    if (tid == 0) {
+        for (int i = 0; i < 4; ++i) mbar_init(t2bar + i, kProjWarps);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
     __syncthreads();
 
     const real_t* psi_b = reinterpret_cast<const real_t*>(p.psi) + (size_t)b * p.band_stride * P;
@@ -297,9 +302,34 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
         rp = row_ptr(plane_ptr(warp), 0);
         load_group(cur, rp, 0);
     }
+    // ---- a5: z contraction of the 8 planes of one round, thread n <- coefficient n ----
+    auto a5 = [&](int rnd) {
+        const double* t2r = t2s + (size_t)(rnd & 3) * kProjWarps * P * TS;
+        const int wmax = min(kProjWarps, nzl - rnd * kProjWarps);
+#pragma unroll
+        for (int j = 0; j < NACC; ++j) {
+            const int n = tid + j * blockDim.x;
+            if (n < p.g.nsho) {
+                for (int w = 0; w < wmax; ++w) {
+                    const int z2 = rnd * kProjWarps + w;
+                    const double f = fz[(size_t)z2 * NV + mynz[j]];
+                    const double* tt = t2r + (size_t)w * P * TS + myt2[j];
+                    if (!CPLX) {
+                        acc[j][0] = fma(f, tt[0], acc[j][0]);
+                    } else {
+                        const double re = tt[0], im = tt[TS];
+                        const double cr = wz[2 * z2], ci = wz[2 * z2 + 1];
+                        acc[j][0] = fma(f, re * cr - im * ci, acc[j][0]);
+                        acc[j][P - 1] = fma(f, re * ci + im * cr, acc[j][P - 1]);
+                    }
+                }
+            }
+        }
+    };
+
     for (int round = 0; round < nrounds; ++round) {
         const int zi = round * kProjWarps + warp;
-        double* t2w = t2s + ((size_t)(round & 1) * kProjWarps + warp) * P * TS;
+        double* t2w = t2s + ((size_t)(round & 3) * kProjWarps + warp) * P * TS;
         if (zi < nzl) {
             const real_t* pz = plane_ptr(zi);
             const real_t* pzn = (zi + kProjWarps < nzl) ? plane_ptr(zi + kProjWarps) : pz;
@@ -502,30 +532,14 @@ __global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const P
                 }
             }
         }
-        __syncthreads();
-        // ---- a5: z contraction, thread n <- coefficient n ----
-        const double* t2r = t2s + (size_t)(round & 1) * kProjWarps * P * TS;
-        const int wmax = min(kProjWarps, nzl - round * kProjWarps);
-#pragma unroll
-        for (int j = 0; j < NACC; ++j) {
-            const int n = tid + j * blockDim.x;
-            if (n < p.g.nsho) {
-                for (int w = 0; w < wmax; ++w) {
-                    const int z2 = round * kProjWarps + w;
-                    const double f = fz[(size_t)z2 * NV + mynz[j]];
-                    const double* tt = t2r + (size_t)w * P * TS + myt2[j];
-                    if (!CPLX) {
-                        acc[j][0] = fma(f, tt[0], acc[j][0]);
-                    } else {
-                        const double re = tt[0], im = tt[TS];
-                        const double cr = wz[2 * z2], ci = wz[2 * z2 + 1];
-                        acc[j][0] = fma(f, re * cr - im * ci, acc[j][0]);
-                        acc[j][P - 1] = fma(f, re * ci + im * cr, acc[j][P - 1]);
-                    }
-                }
-            }
-        }
+        // The planes of this round are handed over through T2 buffer round & 3; its a5 runs one round later,
+        // so a warp waits for the others only when it is more than a whole plane ahead of the slowest.  Buffer
+        // reuse is safe with four: a5(r-4) precedes arrive(r-2) in every warp, and this warp waited for (r-2).
+        __syncwarp();
+        if (lane == 0) mbar_arrive(t2bar + (round & 3));
+        if (round >= 1) { mbar_wait(t2bar + ((round - 1) & 3), ((round - 1) >> 2) & 1); a5(round - 1); }
     }
+    if (nrounds >= 1) { mbar_wait(t2bar + ((nrounds - 1) & 3), ((nrounds - 1) >> 2) & 1); a5(nrounds - 1); }
 
     // ---- store: c[a][b][n] = h^3 * acc (reading A7) ----
     const double h3 = p.g.h * p.g.h * p.g.h;
