@@ -201,6 +201,96 @@ def test_remainder_rows_every_dtype(sho, numax, dtype):
     run_case(sho, w, stored=False)
 
 
+def test_many_pairs_per_tile_wrap_the_ring(sho):
+    # 60 atoms whose boxes all cover the same add tiles: the mbarrier ring of the add kernel (<= 18 pairs)
+    # wraps several times, every producer warp reuses its slots and buffers
+    rng = np.random.default_rng(5)
+    ng = (16, 64, 16)
+    pos = (np.array(ng) * 0.25 / 2)[None, :] + rng.uniform(-0.4, 0.4, (60, 3))
+    run_case(sho, _custom(ng, (1, 1, 1), pos, rng.uniform(0.3, 0.33, 60), 4, 2, rc=5.0), stored=False)
+    run_case(sho, _custom(ng, (1, 1, 1), pos, rng.uniform(0.3, 0.33, 60), 9, 2, dtype="c128", kfrac=(0.1, 0.2, 0.3), rc=5.0),
+             stored=False)
+
+
+@pytest.mark.parametrize("nb", [1, 3])
+def test_odd_number_of_real_bands(sho, nb):
+    # the add kernel pairs real bands into two channels per CTA: the last CTA has an idle channel
+    rng = np.random.default_rng(17)
+    ng = (24, 40, 16)
+    pos = rng.uniform(0, 1, (6, 3)) * np.array(ng) * 0.25
+    run_case(sho, _custom(ng, (1, 1, 1), pos, rng.uniform(0.3, 0.36, 6), 5, nb, rc=4.0), stored=False)
+    run_case(sho, _custom(ng, (1, 1, 1), pos, rng.uniform(0.3, 0.36, 6), 5, nb, dtype="r32", rc=4.0), stored=False)
+
+
+@pytest.mark.parametrize("nx", [18, 22, 36])
+def test_bloch_image_boundary_inside_a_load_step(sho, nx):
+    # complex128, Nx a multiple of the 2-element lane span but not of the 8-column step: the x-image
+    # boundary of a wrapping atom falls inside a step, which the project kernel schedules twice with
+    # complementary column masks around the accumulator rotation
+    rng = np.random.default_rng(nx)
+    ng = (nx, 20, 16)
+    L = np.array(ng) * 0.25
+    pos = np.stack([np.array([0.3, 2.0, 2.0]), np.array([L[0] - 0.2, 3.0, 1.0]), np.array([L[0] / 2, 0.1, 3.9])])
+    run_case(sho, _custom(ng, (1, 1, 1), pos, [0.3, 0.34, 0.32], 9, 2, dtype="c128", kfrac=(0.17, 0.2, 0.3), rc=5.0))
+    run_case(sho, _custom(ng, (1, 1, 1), pos, [0.3, 0.34, 0.32], 6, 3, dtype="c64", kfrac=(0.17, -0.2, 0.3), rc=5.0))
+
+
+@pytest.mark.parametrize("k", [3, 4, 5])
+def test_full_size_config_sampled(sho, k):
+    """BASELINE.json config k at its full size, in the launch configuration bench.py times (all bands, device
+    inputs from a seeded torch generator): project checked on sampled (atom, band) pairs -- atoms whose box
+    wraps on every axis, the smallest and the largest sigma -- and add on 2 z-planes' worth of random points
+    of the first and the last band, each computed one by one by the oracle (reading A13 norms; the add scale
+    is the largest reference increment among the samples)."""
+    import torch
+    w = workloads.make(k)
+    tol = TOL[w.dtype]
+    wide = np.complex128 if w.is_complex else np.float64
+    tdt = {"r64": torch.float64, "c128": torch.complex128, "r32": torch.float32, "c64": torch.complex64}[w.dtype]
+    plan = sho.plan_for(w)
+    try:
+        boxes = _oracle_boxes(w)
+        assert np.array_equal(plan.boxes(), boxes), "integer box ranges differ from the oracle"
+        gen = torch.Generator(device="cuda")
+        gen.manual_seed(w.seed)
+        shape = (w.nbands, w.ng[2], w.ng[1], w.ng[0])
+        psi = torch.randn(shape, dtype=tdt, device="cuda", generator=gen)
+        c_gpu = plan.project(psi)
+        torch.cuda.synchronize()
+        # ---- project: sampled pairs ----
+        ng = np.array(w.ng)
+        wraps = [a for a in range(w.natoms) if all(boxes[a, d, 0] < 0 or boxes[a, d, 1] >= ng[d] for d in range(3))]
+        atoms = sorted(set(wraps[:3] + [int(np.argmin(w.sigma)), int(np.argmax(w.sigma)), 0, w.natoms - 1]))
+        pairs = [(a, b) for a in atoms for b in (0, w.nbands - 1)]
+        bands = {b: psi[b].cpu().numpy().astype(wide) for b in (0, w.nbands - 1)}
+        pa, pb = np.array([q[0] for q in pairs]), np.array([q[1] for q in pairs])
+        ref = oracle.project_pairs(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax, bands, pa, pb, w.nbands,
+                                   w.is_complex, w.rcut_sigma)
+        norm = np.array([np.sqrt(w.h ** 3 * np.sum(np.abs(bands[int(b)]) ** 2)) for b in pb])
+        got = c_gpu[torch.as_tensor(pa, device="cuda"), torch.as_tensor(pb, device="cuda")].cpu().numpy().astype(wide)
+        err = (np.abs(got - ref) / norm[:, None]).max()
+        assert err <= tol, "project parity at full size: %.3e > %.1e" % (err, tol)
+        del psi
+        # ---- add: sampled points ----
+        coeff = torch.randn((w.natoms, w.nbands, plan.nsho), dtype=tdt, device="cuda", generator=gen)
+        out = torch.zeros(shape, dtype=tdt, device="cuda")
+        plan.add(coeff, out)
+        torch.cuda.synchronize()
+        rng = np.random.default_rng(w.seed)
+        ns = 2 * w.ng[0] * w.ng[1] // 8
+        pts = np.stack([rng.integers(0, w.ng[d], ns) for d in range(3)], axis=1)
+        pts[: ns // 4, 2] = 0                       # a quarter of them on the first plane (wrapped boxes)
+        bsel = np.where(rng.integers(0, 2, ns) == 0, 0, w.nbands - 1)
+        refp = oracle.add_points(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax,
+                                 coeff.cpu().numpy().astype(wide), pts, bsel, w.rcut_sigma)
+        gotp = out[torch.as_tensor(bsel, device="cuda"), torch.as_tensor(pts[:, 2], device="cuda"),
+                   torch.as_tensor(pts[:, 1], device="cuda"), torch.as_tensor(pts[:, 0], device="cuda")].cpu().numpy().astype(wide)
+        erra = np.abs(gotp - refp).max() / np.abs(refp).max()
+        assert erra <= tol, "add parity at full size: %.3e > %.1e" % (erra, tol)
+    finally:
+        plan.close()
+
+
 def test_box_exactly_as_wide_as_the_cell(sho):
     # periodic box of exactly N points on x (every grid point once, one wrap)
     ng = (24, 40, 40)
