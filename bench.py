@@ -280,6 +280,32 @@ def run_ours(args, w):
         return 0
 
     fp64_meas = sho.measure_fp64_peak(20000) / 1e12
+    # ---- stored-projector baseline (a7): the same projection from pre-sampled 3D tables in HBM;
+    # outside the timed region of the step.  Tables that do not fit are reported with their size (the capacity wall).
+    stored = None
+    if not args.no_stored:
+        need = plan.tables_bytes()
+        free_b = torch.cuda.mem_get_info(dev)[0]
+        stored = {"table_bytes": need}
+        if need > 0.8 * free_b:
+            stored.update(status="does not fit", free_bytes=int(free_b))
+        else:
+            tb = plan.tables()
+            for _ in range(2):
+                plan.project_stored(tb, psi, coeff, stream)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ks = max(1, min(args.steps, 5))
+            e0.record(stream)
+            for _ in range(ks):
+                plan.project_stored(tb, psi, coeff, stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            t_sto = e0.elapsed_time(e1) * 1e-3 / ks
+            tb.close()
+            stored.update(status="ok", ms_project_stored=1e3 * t_sto, table_gbs=need / t_sto / 1e9,
+                          slowdown_vs_on_the_fly=t_sto / t_prj,
+                          table_bytes_over_psi_box_bytes=need / box_bytes)
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         s = oracle_sample_setup(w, cpu_seconds=args.ref_cpu_seconds)
@@ -302,7 +328,7 @@ def run_ours(args, w):
             "frac_hbm_peak_step": value / world / peaks["hbm_gbs"], "hbm_peak_gbs": peaks["hbm_gbs"], "hbm_peak_kind": peak_kind,
             "atom_band_per_s": world * info["atoms_nonempty"] * nb * args.steps / t_total,
             "tflops_project": F / t_prj / 1e12, "tflops_add": F / t_add / 1e12, "fp64_peak_measured_tflops": fp64_meas,
-            "sum_box_points": g["sum_box"], "psi_bytes_unique": int(np.prod(shape)) * esz, "add_tile_pairs": info["add_pairs"],
+            "stored_baseline": stored, "sum_box_points": g["sum_box"], "psi_bytes_unique": int(np.prod(shape)) * esz, "add_tile_pairs": info["add_pairs"],
         },
     }
     print(json.dumps(line))
@@ -322,6 +348,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-stored", action="store_true", help="skip the stored-projector baseline leg")
     ap.add_argument("--ref-cpu-seconds", type=float, default=20.0)
     args = ap.parse_args()
     w = workloads.make(args.config, dtype=args.dtype)

@@ -115,37 +115,52 @@ __global__ void __launch_bounds__(kStoWarps * 32, 2) sho_project_stored_kernel(c
         for (int k0 = 0; k0 < KP; k0 += kStoKC) {
             const int kc = min(kStoKC, KP - k0);
             __syncthreads();
-            // ---- stage psi (wrap, Bloch phase) as B fragments: B[k = point 4k+t][col = band (x re/im)] ----
-            for (int it = tid; it < (kStoCols / P) * kc * 4; it += blockDim.x) {
-                const int bl = it / (kc * 4), rr = it - bl * (kc * 4);
+            // ---- stage psi (wrap, Bloch phase) as B fragments: B[k = point 4k+t][col = band (x re/im)].  A thread
+            // keeps one point of the chunk (its grid offset and phase are computed once) and walks the bands ----
+            for (int rr = tid; rr < kc * 4; rr += blockDim.x) {
                 const int r = 4 * k0 + rr;
-                double v0 = 0.0, v1 = 0.0;
-                if (bl < nbl && r < npl) {
+                const bool inside = r < npl;
+                size_t j = 0;
+                double cs = 1.0, sn = 0.0;
+                if (inside) {
                     const int qy = r / nxl, qx = r - qy * nxl;
                     const int ix = at.lo[0] + qx, iy = at.lo[1] + qy;
                     const int mx = p.g.periodic[0] ? floordiv(ix, Nx) : 0, my = p.g.periodic[1] ? floordiv(iy, Ny) : 0;
-                    const size_t j = ((size_t)jz * Ny + (iy - my * Ny)) * Nx + (ix - mx * Nx);
-                    const real_t* src = psi + ((size_t)(band0 + bl) * p.band_stride + j) * P;
-                    if (!CPLX) v0 = (double)__ldg(src);
-                    else {
-                        const double re = (double)__ldg(src), im = (double)__ldg(src + 1);
-                        if (p.g.has_phase && (mx | my | mz)) {
-                            double sn, cs;
-                            sincospi(2.0 * (p.g.kfrac[0] * mx + p.g.kfrac[1] * my + p.g.kfrac[2] * mz), &sn, &cs);
-                            v0 = re * cs - im * sn; v1 = re * sn + im * cs;
-                        } else { v0 = re; v1 = im; }
-                    }
+                    j = ((size_t)jz * Ny + (iy - my * Ny)) * Nx + (ix - mx * Nx);
+                    if (CPLX && p.g.has_phase && (mx | my | mz))
+                        sincospi(2.0 * (p.g.kfrac[0] * mx + p.g.kfrac[1] * my + p.g.kfrac[2] * mz), &sn, &cs);
                 }
                 const int kk = rr >> 2, tt = rr & 3;
+                double* dst = bs + kk * kStoKStride + tt;
+                const real_t* src = psi + ((size_t)band0 * p.band_stride + j) * P;
+                constexpr int NB = kStoCols / P;
+                for (int bl0 = 0; bl0 < NB; bl0 += 8) {
+                    double v0[8], v1[8];
 #pragma unroll
-                for (int pp = 0; pp < P; ++pp) {
-                    const int col = bl * P + pp;
-                    bs[kk * kStoKStride + (col >> 3) * 32 + (col & 7) * 4 + tt] = pp ? v1 : v0;
+                    for (int u = 0; u < 8; ++u) {
+                        v0[u] = v1[u] = 0.0;
+                        if (inside && bl0 + u < nbl) {
+                            const real_t* sp = src + (size_t)(bl0 + u) * p.band_stride * P;
+                            v0[u] = (double)__ldg(sp);
+                            if (CPLX) v1[u] = (double)__ldg(sp + 1);
+                        }
+                    }
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        if (!CPLX) {
+                            const int col = bl0 + u;
+                            dst[(col >> 3) * 32 + (col & 7) * 4] = v0[u];
+                        } else {
+                            const int col = (bl0 + u) * 2;
+                            dst[(col >> 3) * 32 + (col & 7) * 4] = v0[u] * cs - v1[u] * sn;
+                            dst[((col + 1) >> 3) * 32 + ((col + 1) & 7) * 4] = v0[u] * sn + v1[u] * cs;
+                        }
+                    }
                 }
             }
             __syncthreads();
             // ---- stream the table fragments, K = 4 points per step ----
-#pragma unroll 2
+#pragma unroll 8
             for (int kk = 0; kk < kc; ++kk) {
                 double afr[MTW];
 #pragma unroll
