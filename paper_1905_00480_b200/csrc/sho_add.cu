@@ -40,12 +40,12 @@ struct AddParams {
     AddZTiles zt;
     const void* coeff;
     void* psi;
-    const int32_t* tile_ptr;
+    const int4* tile_info;     // per listed tile: (tile, first entry, entries, 0)
     const AddEntry* tile_ent;
-    const int32_t* tile_list;
     const uint16_t* cidx;      // [nblk][32] coefficient index held by lane 4 q + t of z-stage K block (0xffff: none)
     const uint16_t* t2pos;
     int32_t n_tile_list;
+    int32_t nitems;            // work items = listed tiles x band chunks (one complex band or two real bands)
     int32_t nbands;
     int32_t ntile0, ntile1;
     int32_t vec_ok;
@@ -58,7 +58,7 @@ struct AddParams {
 };
 
 // shared-memory carve-up (doubles): [FXY: RD x 9 KQ 32][T2: RD x 2 x 8 npp][FZ: npw x KQ 32][STG: npw x stg]
-// [EXPT: 64][ENT: npw x 2 records] then [META: RD int32][ZPOS: 8 nmt uint16][CIDX: 32 nblk uint16][mbarriers: full RD, empty RD]
+// [EXPT: 64][XCH: complex write-back exchange][ENT: npw x 2 records] then [META: RD int32][ZPOS: 8 nmt uint16][CIDX: 32 nblk uint16][mbarriers: full RD, empty RD]
 template <int KQ>
 struct AddSmem {
     static constexpr int FXYS = 9 * KQ * 32;
@@ -66,10 +66,11 @@ struct AddSmem {
     static __host__ __device__ int t2s(int npp) { return 2 * kAddTZ * npp; }
     // z-stage A fragments of one pair in the element type of the data: [K block][lane][channel]
     static __host__ __device__ int stg(int nblk, int real_bytes) { return ((64 * nblk * real_bytes + 15) / 16) * 2; }
-    static __host__ __device__ size_t bytes(int rd, int npw, int nmt, int nblk, int real_bytes)
+    static __host__ __device__ size_t bytes(int rd, int npw, int nmt, int nblk, int real_bytes, bool cplx)
     {
         const int npp = 8 * nmt + 2;
-        size_t b = 8 * ((size_t)rd * (FXYS + t2s(npp)) + (size_t)npw * (FZS + stg(nblk, real_bytes)) + 64);
+        size_t b = 8 * ((size_t)rd * (FXYS + t2s(npp)) + (size_t)npw * (FZS + stg(nblk, real_bytes)) + 64 +
+                        (cplx ? (size_t)kAddTZ * kAddTY * kAddTX : 0));
         b += (size_t)npw * 2 * sizeof(AddEntry);
         b += (size_t)rd * 4 + (size_t)8 * nmt * 2 + (size_t)32 * nblk * 2;
         b = (b + 7) & ~(size_t)7;
@@ -158,7 +159,8 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
     double* FZ = T2 + (size_t)RD * T2S;                   // [npw][KQ][32]
     double* STG = FZ + (size_t)NPW * FZS;                 // [npw][STGS]   z-stage A fragments of the pair in production, element type of the data
     double* EXPT = STG + (size_t)NPW * STGS;              // [64]  2^(j/64), see exp_neg
-    AddEntry* ENTW = reinterpret_cast<AddEntry*>(EXPT + 64);                     // [npw][2]  this and the next record
+    double* XCH = EXPT + 64;                              // complex only: [8 planes][64 x 8] imaginary parts on their way out
+    AddEntry* ENTW = reinterpret_cast<AddEntry*>(XCH + (CPLX ? kAddTZ * kAddTY * kAddTX : 0));                     // [npw][2]  this and the next record
     int32_t* META = reinterpret_cast<int32_t*>(ENTW + 2 * NPW);                  // [RD] zmask | ytlo << 8 | ythi << 16
     uint16_t* ZPOS = reinterpret_cast<uint16_t*>(META + RD);                     // [8 nmt] T2 column of z-stage row
     uint16_t* CIDX = ZPOS + 8 * nmt;                                             // [nblk][32] coefficient of an A-fragment element
@@ -168,15 +170,26 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int q = lane >> 2, t = lane & 3;
 
-    // work item: tile x band chunk (one complex band or two real bands), chunk-major
-    const int chunk = blockIdx.x / p.n_tile_list;
-    const int tile = p.tile_list[blockIdx.x - chunk * p.n_tile_list];
-    const int b0 = CPLX ? chunk : 2 * chunk;
-    const int tx = tile % p.ntile0, ty = (tile / p.ntile0) % p.ntile1, tz = tile / (p.ntile0 * p.ntile1);
-    const int jx0 = tx * kAddTX, jy0 = ty * kAddTY, jz0 = tz * kAddTZ;
+    // The CTA is persistent: it takes work items blockIdx.x, blockIdx.x + gridDim.x, ... (item = band chunk x
+    // listed tile, tile fastest; a chunk is one complex band or two real bands) and the ring runs on across
+    // them, so the producers fill it for the next tile while the XY warps write the finished one back.
     const int Nx = p.g.ng[0], Ny = p.g.ng[1], Nz = p.g.ng[2];
-    const int ebeg = p.tile_ptr[tile], eend = p.tile_ptr[tile + 1];
-    const int npairs = eend - ebeg;
+    struct Item { int b0, jx0, jy0, jz0, ebeg, npairs; };
+    auto item_info = [&](int item) -> int4 {          // (tile, first entry, entries, chunk)
+        const int chunk = item / p.n_tile_list;
+        int4 v = __ldg(p.tile_info + (item - chunk * p.n_tile_list));
+        v.w = chunk;
+        return v;
+    };
+    auto decode = [&](const int4& v) -> Item {
+        Item it;
+        it.b0 = CPLX ? v.w : 2 * v.w;
+        const int tile = v.x;
+        const int tx = tile % p.ntile0, ty = (tile / p.ntile0) % p.ntile1, tz = tile / (p.ntile0 * p.ntile1);
+        it.jx0 = tx * kAddTX; it.jy0 = ty * kAddTY; it.jz0 = tz * kAddTZ;
+        it.ebeg = v.y; it.npairs = v.z;
+        return it;
+    };
 
     // zero T2 once: its zero column stays zero (z-stage rows past the last pair write zeros there)
     for (int i = tid; i < RD * T2S; i += kAddThreads) T2[i] = 0.0;
@@ -192,24 +205,6 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
     if (warp < kAddXYWarps) {
         // =============================== XY warps ===============================
         const int plane = warp & 7, ch = warp >> 3;
-        const bool active = CPLX || (b0 + ch < p.nbands);
-        const int jz = jz0 + plane;
-        real_t* pb = reinterpret_cast<real_t*>(p.psi) +
-                     (CPLX ? ((size_t)b0 * p.band_stride + (size_t)jz * Ny * Nx) * 2 + ch
-                           : ((size_t)(b0 + ch) * p.band_stride + (size_t)jz * Ny * Nx));
-        // the owned rows are read once, at the very end: ask L2 for their lines now
-        if (active && npairs > 0 && jz < Nz && (!CPLX || ch == 0)) {
-            constexpr int kLineElems = 128 / (int)(sizeof(real_t) * P);           // tile columns per 128-byte line
-            for (int r = lane; r < kAddTY * ((kAddTX + kLineElems - 1) / kLineElems); r += 32) {
-                const int row = r % kAddTY, seg = r / kAddTY;
-                if (jy0 + row < Ny && jx0 + seg * kLineElems < Nx)
-                    asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + ((size_t)(jy0 + row) * Nx + jx0 + seg * kLineElems) * P));
-            }
-        }
-
-        double D[NYT][2];
-#pragma unroll
-        for (int yt = 0; yt < NYT; ++yt) D[yt][0] = D[yt][1] = 0.0;
         // x stage, B fragment B[k = nx][col = ny]: this lane reads T2[(ny,nx)] with nx = 4 ks + t and
         // ny = 8 nt + 4 (q & 1) + (q >> 1); pairs outside the basis read the zero column
         int t2off[NT][KQ];
@@ -221,101 +216,125 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
         int slot = 0, ph = 0;
         const double* fxy = FXY + lane;
         const double* t2p = T2 + (size_t)(ch * kAddTZ + plane) * npp;
-        for (int g = 0; g < npairs; ++g) {
-            mbar_wait(full + slot, ph);
-            const int meta = META[slot];
-            if (active && ((meta >> plane) & 1)) {
-                const int ytlo = (meta >> 8) & 0xff, ythi = (meta >> 16) & 0xff;
-                double D1[NT][2];
+        int4 info_next = item_info(blockIdx.x);
+        for (int item = blockIdx.x; item < p.nitems; item += gridDim.x) {
+            const Item it = decode(info_next);
+            if (item + (int)gridDim.x < p.nitems) info_next = item_info(item + gridDim.x);   // arrives during this item
+            const int npairs = it.npairs;
+            const bool active = CPLX || (it.b0 + ch < p.nbands);
+            const int jz = it.jz0 + plane;
+            real_t* pb = reinterpret_cast<real_t*>(p.psi) +
+                         (CPLX ? ((size_t)it.b0 * p.band_stride + (size_t)jz * Ny * Nx) * 2
+                               : ((size_t)(it.b0 + ch) * p.band_stride + (size_t)jz * Ny * Nx));
+            // the owned rows are read once, at the end of the item: ask L2 for their lines now
+            if (active && jz < Nz && (!CPLX || ch == 0)) {
+                constexpr int kLineElems = 128 / (int)(sizeof(real_t) * P);           // tile columns per 128-byte line
+                for (int r = lane; r < kAddTY * ((kAddTX + kLineElems - 1) / kLineElems); r += 32) {
+                    const int row = r % kAddTY, seg = r / kAddTY;
+                    if (it.jy0 + row < Ny && it.jx0 + seg * kLineElems < Nx)
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + ((size_t)(it.jy0 + row) * Nx + it.jx0 + seg * kLineElems) * P));
+                }
+            }
+            double D[NYT][2];
 #pragma unroll
-                for (int nt = 0; nt < NT; ++nt) D1[nt][0] = D1[nt][1] = 0.0;
-                // independent accumulators next to each other: a dependent DMMA issues 26 cycles after its source
+            for (int yt = 0; yt < NYT; ++yt) D[yt][0] = D[yt][1] = 0.0;
+
+            for (int g = 0; g < npairs; ++g) {
+                mbar_wait(full + slot, ph);
+                const int meta = META[slot];
+                if (active && ((meta >> plane) & 1)) {
+                    const int ytlo = (meta >> 8) & 0xff, ythi = (meta >> 16) & 0xff;
+                    double D1[NT][2];
 #pragma unroll
-                for (int ks = 0; ks < KQ; ++ks)
+                    for (int nt = 0; nt < NT; ++nt) D1[nt][0] = D1[nt][1] = 0.0;
+                    // independent accumulators next to each other: a dependent DMMA issues 26 cycles after its source
 #pragma unroll
-                    for (int nt = 0; nt < NT; ++nt)
-                        if (8 * nt + 4 * ks <= 4 * KQ - 4)                  // the block holds some ny+nx <= numax (numax >= 4 KQ - 4)
-                            dmma(D1[nt][0], D1[nt][1], fxy[(8 * KQ + ks) * 32], t2p[t2off[nt][ks]]);
-                // The touched 8-row blocks are ytlo..ythi.  A predicated-off DMMA still takes its 16 cycles of the
-                // pipe (measured), and the compiler predicates a short "if": enter the unrolled blocks by a jump
-                // and leave them by a branch instead.
+                    for (int ks = 0; ks < KQ; ++ks)
+#pragma unroll
+                        for (int nt = 0; nt < NT; ++nt)
+                            if (8 * nt + 4 * ks <= 4 * KQ - 4)              // the block holds some ny+nx <= numax (numax >= 4 KQ - 4)
+                                dmma(D1[nt][0], D1[nt][1], fxy[(8 * KQ + ks) * 32], t2p[t2off[nt][ks]]);
+                    // The touched 8-row blocks are ytlo..ythi.  A predicated-off DMMA still takes its 16 cycles of
+                    // the pipe (measured), and the compiler predicates a short "if": enter the unrolled blocks by
+                    // a jump and leave them by a branch instead.
 #define SHO_ADD_YBLOCK(YT)                                                                              \
     {                                                                                                   \
         double a_[KQ];                                                                                  \
         _Pragma("unroll") for (int kk = 0; kk < KQ; ++kk) a_[kk] = fxy[((YT) * KQ + kk) * 32];          \
         _Pragma("unroll") for (int kk = 0; kk < KQ; ++kk) dmma(D[YT][0], D[YT][1], a_[kk], D1[kk >> 1][kk & 1]); \
     }
-                switch (ytlo) {
-                    case 0: SHO_ADD_YBLOCK(0) if (ythi == 0) break;
-                    case 1: SHO_ADD_YBLOCK(1) if (ythi == 1) break;
-                    case 2: SHO_ADD_YBLOCK(2) if (ythi == 2) break;
-                    case 3: SHO_ADD_YBLOCK(3) if (ythi == 3) break;
-                    case 4: SHO_ADD_YBLOCK(4) if (ythi == 4) break;
-                    case 5: SHO_ADD_YBLOCK(5) if (ythi == 5) break;
-                    case 6: SHO_ADD_YBLOCK(6) if (ythi == 6) break;
-                    case 7: SHO_ADD_YBLOCK(7)
-                    default: break;
-                }
+                    switch (ytlo) {
+                        case 0: SHO_ADD_YBLOCK(0) if (ythi == 0) break;
+                        case 1: SHO_ADD_YBLOCK(1) if (ythi == 1) break;
+                        case 2: SHO_ADD_YBLOCK(2) if (ythi == 2) break;
+                        case 3: SHO_ADD_YBLOCK(3) if (ythi == 3) break;
+                        case 4: SHO_ADD_YBLOCK(4) if (ythi == 4) break;
+                        case 5: SHO_ADD_YBLOCK(5) if (ythi == 5) break;
+                        case 6: SHO_ADD_YBLOCK(6) if (ythi == 6) break;
+                        case 7: SHO_ADD_YBLOCK(7)
+                        default: break;
+                    }
 #undef SHO_ADD_YBLOCK
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(empty + slot);
-            fxy += FXYS; t2p += T2S;
-            if (++slot == RD) { slot = 0; ph ^= 1; fxy = FXY + lane; t2p = T2 + (size_t)(ch * kAddTZ + plane) * npp; }
-        }
-
-        // ---------------- one read-modify-write of the owned rows ----------------
-        if (CPLX) {
-            // the warp of the imaginary part hands its accumulators to the warp of the real part through the
-            // (now idle) ring, so that psi is read and written as whole complex numbers
-            asm volatile("bar.sync 1, %0;\n" ::"r"(kAddXYWarps * 32) : "memory");      // every XY warp is done with the ring
-            double* xch = smem + (size_t)plane * (kAddTY * kAddTX);
-            if (ch == 1) {
-#pragma unroll
-                for (int yt = 0; yt < NYT; ++yt) {
-                    double2 v; v.x = D[yt][0]; v.y = D[yt][1];
-                    *reinterpret_cast<double2*>(xch + (8 * yt + q) * kAddTX + 2 * t) = v;
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + slot);
+                fxy += FXYS; t2p += T2S;
+                if (++slot == RD) { slot = 0; ph ^= 1; fxy = FXY + lane; t2p = T2 + (size_t)(ch * kAddTZ + plane) * npp; }
             }
-            asm volatile("bar.sync 1, %0;\n" ::"r"(kAddXYWarps * 32) : "memory");
-            if (ch == 0 && jz < Nz && npairs > 0) {
-                const int jx = jx0 + 2 * t;
+
+            // ---------------- one read-modify-write of the owned rows ----------------
+            if (CPLX) {
+                // the warp of the imaginary part hands its accumulators to the warp of the real part through
+                // shared memory, so that psi is read and written as whole complex numbers
+                double* xch = XCH + (size_t)plane * (kAddTY * kAddTX);
+                if (ch == 1) {
 #pragma unroll
-                for (int yt = 0; yt < NYT; ++yt) {
-                    const int jy = jy0 + 8 * yt + q;
-                    const double2 im = *reinterpret_cast<const double2*>(xch + (8 * yt + q) * kAddTX + 2 * t);
-                    if (jy < Ny) {
-                        real_t* pc = pb + ((size_t)jy * Nx + jx) * 2;
-#pragma unroll
-                        for (int sx = 0; sx < 2; ++sx)
-                            if (jx + sx < Nx) {
-                                const double dre = D[yt][sx], dim = sx ? im.y : im.x;
-                                if (p.vec_ok) {
-                                    double v0, v1;
-                                    load2_rw(pc + 2 * sx, v0, v1);
-                                    store2(pc + 2 * sx, v0 + dre, v1 + dim);
-                                } else {
-                                    pc[2 * sx] = (real_t)((double)pc[2 * sx] + dre);
-                                    pc[2 * sx + 1] = (real_t)((double)pc[2 * sx + 1] + dim);
-                                }
-                            }
+                    for (int yt = 0; yt < NYT; ++yt) {
+                        double2 v; v.x = D[yt][0]; v.y = D[yt][1];
+                        *reinterpret_cast<double2*>(xch + (8 * yt + q) * kAddTX + 2 * t) = v;
                     }
                 }
-            }
-        } else if (active && jz < Nz && npairs > 0) {
-            const int jx = jx0 + 2 * t;
+                asm volatile("bar.sync 1, %0;\n" ::"r"(kAddXYWarps * 32) : "memory");
+                if (ch == 0 && jz < Nz) {
+                    const int jx = it.jx0 + 2 * t;
 #pragma unroll
-            for (int yt = 0; yt < NYT; ++yt) {
-                const int jy = jy0 + 8 * yt + q;
-                if (jy < Ny && jx < Nx) {
-                    real_t* pp_ = pb + ((size_t)jy * Nx + jx);
-                    if (p.vec_ok && jx + 1 < Nx) {
-                        double v0, v1;
-                        load2_rw(pp_, v0, v1);
-                        store2(pp_, v0 + D[yt][0], v1 + D[yt][1]);
-                    } else {
-                        pp_[0] = (real_t)((double)pp_[0] + D[yt][0]);
-                        if (jx + 1 < Nx) pp_[1] = (real_t)((double)pp_[1] + D[yt][1]);
+                    for (int yt = 0; yt < NYT; ++yt) {
+                        const int jy = it.jy0 + 8 * yt + q;
+                        const double2 im = *reinterpret_cast<const double2*>(xch + (8 * yt + q) * kAddTX + 2 * t);
+                        if (jy < Ny) {
+                            real_t* pc = pb + ((size_t)jy * Nx + jx) * 2;
+#pragma unroll
+                            for (int sx = 0; sx < 2; ++sx)
+                                if (jx + sx < Nx) {
+                                    const double dre = D[yt][sx], dim = sx ? im.y : im.x;
+                                    if (p.vec_ok) {
+                                        double v0, v1;
+                                        load2_rw(pc + 2 * sx, v0, v1);
+                                        store2(pc + 2 * sx, v0 + dre, v1 + dim);
+                                    } else {
+                                        pc[2 * sx] = (real_t)((double)pc[2 * sx] + dre);
+                                        pc[2 * sx + 1] = (real_t)((double)pc[2 * sx + 1] + dim);
+                                    }
+                                }
+                        }
+                    }
+                }
+                asm volatile("bar.sync 1, %0;\n" ::"r"(kAddXYWarps * 32) : "memory");     // the exchange buffer is free again
+            } else if (active && jz < Nz) {
+                const int jx = it.jx0 + 2 * t;
+#pragma unroll
+                for (int yt = 0; yt < NYT; ++yt) {
+                    const int jy = it.jy0 + 8 * yt + q;
+                    if (jy < Ny && jx < Nx) {
+                        real_t* pp_ = pb + ((size_t)jy * Nx + jx);
+                        if (p.vec_ok && jx + 1 < Nx) {
+                            double v0, v1;
+                            load2_rw(pp_, v0, v1);
+                            store2(pp_, v0 + D[yt][0], v1 + D[yt][1]);
+                        } else {
+                            pp_[0] = (real_t)((double)pp_[0] + D[yt][0]);
+                            if (jx + 1 < Nx) pp_[1] = (real_t)((double)pp_[1] + D[yt][1]);
+                        }
                     }
                 }
             }
@@ -326,29 +345,48 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
         // pair may be NPW times the XY warps' time per pair before they starve.  Global latency never sits on
         // that path: the pair's raw coefficients are copied to shared memory by cp.async while the tables are
         // sampled, and the record of the warp's next pair while this one is produced.
+        // The pairs of all of this CTA's work items form one stream; warp pw takes elements pw, pw + NPW, ...
         const int pw = warp - kAddXYWarps;
-        if (pw < NPW && pw < npairs) {
+        if (pw < NPW) {
         double* fzw = FZ + (size_t)pw * FZS;
         real_t* stg = reinterpret_cast<real_t*>(STG + (size_t)pw * STGS);
         AddEntry* entw = ENTW + 2 * pw;
-        const real_t* cbase = reinterpret_cast<const real_t*>(p.coeff) + (size_t)b0 * nsho * P;
         const size_t catom = (size_t)p.nbands * nsho * P;
-        const bool two = CPLX || (b0 + 1 < p.nbands);      // second channel exists
         // copy granule: one complex coefficient when its alignment is known, else one real number
         const int gran = (CPLX && p.vec_ok) ? 2 : 1;       // reals per cp.async
-        auto fetch_entry = [&](int g, int buf) {
-            if (lane < 6 && g < npairs)
-                cp_async(reinterpret_cast<char*>(entw + buf) + 16 * lane,
-                         reinterpret_cast<const char*>(p.tile_ent + ebeg + g) + 16 * lane, 16);
+        // stream cursor: (citem, ci) is the work item that holds stream element cbase_s .. cbase_s + ci.z - 1;
+        // the record of the item after it is already on its way (pf)
+        const int grid = (int)gridDim.x;
+        int citem = blockIdx.x, cbase_s = 0;
+        int4 ci = item_info(citem);
+        int4 pf = (citem + grid < p.nitems) ? item_info(citem + grid) : make_int4(0, 0, 0, 0);
+        auto seek = [&](int gs) -> bool {
+            while (citem < p.nitems && gs >= cbase_s + ci.z) {
+                cbase_s += ci.z;
+                citem += grid;
+                ci = pf;
+                if (citem + grid < p.nitems) pf = item_info(citem + grid);
+            }
+            return citem < p.nitems;
         };
-        fetch_entry(pw, 0);
-        asm volatile("cp.async.wait_all;\n" ::: "memory");
-        __syncwarp();
+        auto fetch_entry = [&](int gs, int buf) {        // the cursor stands on stream element gs
+            if (lane < 6)
+                cp_async(reinterpret_cast<char*>(entw + buf) + 16 * lane,
+                         reinterpret_cast<const char*>(p.tile_ent + ci.y + (gs - cbase_s)) + 16 * lane, 16);
+        };
+        int G = pw;
+        bool more = seek(G);
+        if (more) fetch_entry(G, 0);
+        int4 cur = ci;
         int slot = pw % RD, k = pw / RD, ebuf = 0;
-        for (int g = pw; g < npairs; g += NPW, ebuf ^= 1) {
+        for (; more; G += NPW, ebuf ^= 1) {
             asm volatile("cp.async.wait_all;\n" ::: "memory");           // this pair's record (issued one iteration ago)
             __syncwarp();
             const AddEntry* en = entw + ebuf;
+            const Item it = decode(cur);
+            const int jx0 = it.jx0, jy0 = it.jy0, jz0 = it.jz0;
+            const real_t* cbase = reinterpret_cast<const real_t*>(p.coeff) + (size_t)it.b0 * nsho * P;
+            const bool two = CPLX || (it.b0 + 1 < p.nbands);      // second channel exists
             // ---- coefficients of the pair -> A fragments of the z stage.  Every coefficient sits in exactly one
             // fragment element: the lane copies its own (cp.async gather, zero fill for the padding elements) ----
             {
@@ -366,8 +404,10 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
                 }
             }
             asm volatile("cp.async.commit_group;\n" ::: "memory");
-            fetch_entry(g + NPW, ebuf ^ 1);                          // not waited for before the next iteration
+            more = seek(G + NPW);                                    // the cursor moves on to this warp's next pair
+            if (more) fetch_entry(G + NPW, ebuf ^ 1);                // not waited for before the next iteration
             asm volatile("cp.async.commit_group;\n" ::: "memory");
+            cur = ci;
             const double inv_sigma = en->inv_sigma, pref = en->pref;
             const int ytlo = en->ytlo, ythi = en->ythi;
             if (k >= 1) mbar_wait(empty + slot, (k - 1) & 1);        // the slot's previous pair has been consumed
@@ -465,7 +505,7 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
     p.g = pl->g;
     p.zt = pl->ztiles;
     p.coeff = coeff; p.psi = psi;
-    p.tile_ptr = pl->d_tile_ptr; p.tile_ent = pl->d_tile_ent; p.tile_list = pl->d_tile_list;
+    p.tile_info = pl->d_tile_info; p.tile_ent = pl->d_tile_ent;
     p.cidx = pl->d_cidx; p.t2pos = pl->d_t2pos;
     p.n_tile_list = pl->n_tile_list;
     p.nbands = nbands;
@@ -484,15 +524,11 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
     const int rb = (int)(esz / (CPLX ? 2 : 1));
     const size_t budget = 224 * 1024;
     int npw = kAddPWarps;
-    while (npw > 1 && S::bytes(npw + 2, npw, zt.nmt, zt.nblk, rb) > budget) --npw;
+    while (npw > 1 && S::bytes(npw + 2, npw, zt.nmt, zt.nblk, rb, CPLX) > budget) --npw;
     int rd = npw + 2;
-    while (rd < 2 * npw + 2 && S::bytes(rd + 1, npw, zt.nmt, zt.nblk, rb) <= budget) ++rd;
+    while (rd < 2 * npw + 2 && S::bytes(rd + 1, npw, zt.nmt, zt.nblk, rb, CPLX) <= budget) ++rd;
     p.npw = npw; p.rd = rd;
-    if (CPLX && (size_t)rd * (S::FXYS + S::t2s(p.npp)) < (size_t)kAddTZ * kAddTY * kAddTX) {
-        set_error("sho_add: ring too small for the complex write-back exchange");
-        return SHO_ERR_UNSUPPORTED;
-    }
-    const size_t smem = S::bytes(rd, npw, zt.nmt, zt.nblk, rb);
+    const size_t smem = S::bytes(rd, npw, zt.nmt, zt.nblk, rb, CPLX);
     if (smem > 227 * 1024) {
         set_error("sho_add: numax = %d needs %zu bytes of shared memory (> 227 KB)", pl->g.numax, smem);
         return SHO_ERR_UNSUPPORTED;
@@ -501,9 +537,14 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(add)");
     const int nchunk = CPLX ? nbands : (nbands + 1) / 2;
-    const long long nblocks = (long long)pl->n_tile_list * nchunk;
-    if (nblocks > 0x7fffffffLL) { set_error("sho_add: tiles*nbands too large"); return SHO_ERR_UNSUPPORTED; }
-    kern<<<(unsigned)nblocks, kAddThreads, smem, s>>>(p);
+    const long long nitems = (long long)pl->n_tile_list * nchunk;
+    if (nitems > 0x7fffffffLL) { set_error("sho_add: tiles*nbands too large"); return SHO_ERR_UNSUPPORTED; }
+    p.nitems = (int)nitems;
+    int nsm = 0;
+    e = cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, pl->device);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute(add)");
+    const unsigned grid = (unsigned)std::min<long long>(nitems, std::max(nsm, 1));     // persistent: one CTA per SM
+    kern<<<grid, kAddThreads, smem, s>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "launch sho_add_kernel");
     return SHO_OK;

@@ -52,10 +52,10 @@ static sho_status upload(T** dst, const std::vector<T>& src, const char* what)
 static void plan_free_device(sho_plan* p)
 {
     cudaFree(p->d_atoms); cudaFree(p->d_order); cudaFree(p->d_nxyz);
-    cudaFree(p->d_tile_ptr); cudaFree(p->d_tile_ent); cudaFree(p->d_tile_list); cudaFree(p->d_cainv); cudaFree(p->d_t2pos); cudaFree(p->d_cidx);
+    cudaFree(p->d_tile_ptr); cudaFree(p->d_tile_ent); cudaFree(p->d_tile_list); cudaFree(p->d_tile_info); cudaFree(p->d_cainv); cudaFree(p->d_t2pos); cudaFree(p->d_cidx);
     cudaFree(p->ws_psi); cudaFree(p->ws_c);
     p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr; p->d_cidx = nullptr;
-    p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr;
+    p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr; p->d_tile_info = nullptr;
     p->ws_psi = nullptr; p->ws_c = nullptr;
 }
 
@@ -122,7 +122,7 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
     sho_plan* p = new (std::nothrow) sho_plan();
     if (!p) { set_error("sho_plan_create: host allocation failed"); return SHO_ERR_OOM; }
     p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr;
-    p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr; p->d_cidx = nullptr;
+    p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr; p->d_tile_info = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr; p->d_cidx = nullptr;
     p->ws_psi = nullptr; p->ws_c = nullptr; p->ws_psi_bytes = 0; p->ws_c_bytes = 0;
     p->rcut_sigma = rcut_sigma;
     p->dtype = dtype;
@@ -301,6 +301,8 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
     for (int64_t t = 0; t < p->ntiles; ++t)
         if (tile_ptr[t + 1] > tile_ptr[t]) tile_list.push_back((int32_t)t);
     p->n_tile_list = (int32_t)tile_list.size();
+    std::vector<int4> tile_info;
+    for (int32_t t : tile_list) tile_info.push_back(make_int4(t, tile_ptr[(size_t)t], tile_ptr[(size_t)t + 1] - tile_ptr[(size_t)t], 0));
 
     // ---- z stage of the add as an MMA: (ny,nx) pairs sorted by s = ny+nx, row tiles of 8 ----
     std::vector<uint16_t> cainv((size_t)g.nsho, 0);
@@ -362,6 +364,7 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
         (st = upload(&p->d_tile_ptr, tile_ptr, "sho_plan_create: tile_ptr")) != SHO_OK ||
         (st = upload(&p->d_tile_ent, tile_ent, "sho_plan_create: tile_ent")) != SHO_OK ||
         (st = upload(&p->d_tile_list, tile_list, "sho_plan_create: tile_list")) != SHO_OK ||
+        (st = upload(&p->d_tile_info, tile_info, "sho_plan_create: tile_info")) != SHO_OK ||
         (st = upload(&p->d_cainv, cainv, "sho_plan_create: cainv")) != SHO_OK ||
         (st = upload(&p->d_t2pos, t2pos, "sho_plan_create: t2pos")) != SHO_OK ||
         (st = upload(&p->d_cidx, cidx, "sho_plan_create: cidx")) != SHO_OK) {

@@ -88,6 +88,7 @@ struct sho_plan {
     int32_t* d_tile_ptr;                   // [ntiles+1]
     sho::AddEntry* d_tile_ent;             // [npairs]
     int32_t* d_tile_list;                  // tiles with at least one entry
+    int4* d_tile_info;                     // per listed tile: (tile, first entry, entries, 0): one 16-byte load per work item
     int32_t n_tile_list;
     sho::AddZTiles ztiles;
     uint16_t* d_cainv;                     // [nsho] coefficient n -> slot (block*32 + 4 q + t) of the z-stage A fragments
