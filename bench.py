@@ -240,11 +240,11 @@ def run_ours(args, w):
     dom, t_dom = ("sho_add_kernel", t_add) if t_add >= t_prj else ("sho_project_kernel", t_prj)
     alu_peak = FP64_PEAK_TFLOPS                                      # arithmetic is fp64 for all four dtypes
     # dram__bytes_read + dram__bytes_write of one launch from the committed ncu --set full capture (cfg5 only)
-    traffic = {"sho_add_kernel": 8.356264e9 + 7.197572e9, "sho_project_kernel": 9.586075e9 + 0.260884e9}.get(dom) \
+    traffic = {"sho_add_kernel": 8.292317e9 + 7.196499e9, "sho_project_kernel": 9.515675e9 + 0.237247e9}.get(dom) \
         if (w.name == "cfg5" and w.dtype == "c128") else None
     roofline = {"bound": "alu", "kernel": dom, "achieved": F / t_dom / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
                 "frac": F / t_dom / 1e12 / alu_peak, "traffic": traffic,
-                "traffic_source": "profiles/r1_v9_cfg5_ncu_full.txt (bytes per launch)" if traffic else None,
+                "traffic_source": "profiles/r1_final_cfg5_ncu_full.txt (bytes per launch)" if traffic else None,
                 "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md); DMMA/DFMA micro-benchmark in fp64_peak_measured_tflops",
                 "flops_per_launch": F}
 
