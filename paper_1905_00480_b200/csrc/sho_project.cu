@@ -104,7 +104,8 @@ __device__ __forceinline__ void ldg256(const float* p, float (&r)[8])
 }
 
 template <int MT, int R, int DT, int G>
-__global__ void __launch_bounds__(kProjWarps * 32, 2) sho_project_kernel(const ProjParams p)
+// three CTAs per SM for real data (80 registers; measured faster), two for complex data (128 registers)
+__global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_C64 || MT == 2) ? 2 : 3) sho_project_kernel(const ProjParams p)
 {
     using E = Elem<DT>;
     using S = ProjSmem<MT, R, DT>;
