@@ -447,9 +447,6 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
             __syncwarp();
             // ---- z stage: T2[z][(ny,nx)] for the 8 planes; two row tiles in flight ----
             {
-                double bz[KQ];
-#pragma unroll
-                for (int ks = 0; ks < KQ; ++ks) bz[ks] = fzw[ks * 32 + lane];       // B[k = nz][col = plane]
                 const double wr = en->wr, wi = en->wi;
                 const bool phased = !(wr == 1.0 && wi == 0.0);                  // warp-uniform; most images have none
                 double* t2 = T2 + (size_t)slot * T2S + (size_t)(2 * t) * npp;
@@ -461,22 +458,29 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
                         nks[u] = (mt0 + u < nmt) ? p.zt.nks[mt0 + u] : 0;
                         d[u][0][0] = d[u][0][1] = d[u][1][0] = d[u][1][1] = 0.0;
                     }
-#pragma unroll
-                    for (int ks = 0; ks < KQ; ++ks)
-#pragma unroll
-                        for (int u = 0; u < 2; ++u)
-                            if (ks < nks[u]) {                                    // warp-uniform
-                                const real_t* ap = stg + (size_t)((p.zt.blk0[mt0 + u] + ks) * 32 + lane) * 2;
-                                double a0, a1;
-                                load2_rw(ap, a0, a1);
-                                if (CPLX && phased) {                             // conjugate Bloch phase of the image
-                                    const double re = a0, im = a1;
-                                    a0 = re * wr - im * wi;
-                                    a1 = re * wi + im * wr;
-                                }
-                                dmma(d[u][0][0], d[u][0][1], a0, bz[ks]);
-                                dmma(d[u][1][0], d[u][1][1], a1, bz[ks]);
-                            }
+                    auto zstep = [&](int u, int ks, double bzk) {
+                        const real_t* ap = stg + (size_t)((p.zt.blk0[mt0 + u] + ks) * 32 + lane) * 2;
+                        double a0, a1;
+                        load2_rw(ap, a0, a1);
+                        if (CPLX && phased) {                                 // conjugate Bloch phase of the image
+                            const double re = a0, im = a1;
+                            a0 = re * wr - im * wi;
+                            a1 = re * wi + im * wr;
+                        }
+                        dmma(d[u][0][0], d[u][0][1], a0, bzk);
+                        dmma(d[u][1][0], d[u][1][1], a1, bzk);
+                    };
+                    // the tiles are sorted by ny+nx, so nks[0] >= nks[1]: K steps of both, then of the first alone,
+                    // in loops with run-time bounds (real branches: a predicated-off DMMA still costs its pipe time)
+                    int ks = 0;
+#pragma unroll 1
+                    for (; ks < nks[1]; ++ks) {
+                        const double bzk = fzw[ks * 32 + lane];                  // B[k = nz][col = plane]
+                        zstep(0, ks, bzk);
+                        zstep(1, ks, bzk);
+                    }
+#pragma unroll 1
+                    for (; ks < nks[0]; ++ks) zstep(0, ks, fzw[ks * 32 + lane]);
 #pragma unroll
                     for (int u = 0; u < 2; ++u)
                         if (nks[u] > 0) {
