@@ -216,6 +216,17 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
         });
     }
     p->n_nonempty = (int32_t)nonempty.size();
+    {   // x load steps of the project kernel per row block (one 128-byte line per row and step, real data)
+        const int cwx = (dtype == SHO_R32) ? 32 : 16;
+        int64_t steps = 0, odd = 0;
+        for (int a : nonempty) {
+            const AtomDev& at = p->atoms[(size_t)a];
+            const int xs0 = floordiv_h(at.lo[0], cwx) * cwx;
+            const int ks = (at.hi[0] - xs0 + cwx) / cwx;
+            steps += ks; odd += ks & 1;
+        }
+        p->proj_odd_steps = steps ? (double)odd / (double)steps : 0.0;
+    }
     p->order = nonempty;
     p->order.insert(p->order.end(), empty.begin(), empty.end());
 

@@ -565,7 +565,7 @@ __global__ void sho_zero_empty_kernel(T* coeff, const int32_t* order, int first,
     (void)count;
 }
 
-template <int MT, int R, int DT>
+template <int MT, int R, int DT, int G>
 static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s)
 {
     using S = ProjSmem<MT, R, DT>;
@@ -588,7 +588,7 @@ static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void
                   pl->max_n[0], pl->max_n[1], pl->max_n[2], smem);
         return SHO_ERR_UNSUPPORTED;
     }
-    auto kern = sho_project_kernel<MT, R, DT, kProjG>;
+    auto kern = sho_project_kernel<MT, R, DT, G>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(project)");
     const long long nblocks = (long long)pl->n_nonempty * nbands;
@@ -610,14 +610,24 @@ static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void
     return SHO_OK;
 }
 
-template <int DT>
-static sho_status launch_m(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s)
+template <int DT, int G>
+static sho_status launch_mg(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s)
 {
     // numax + 1 functions per axis: <= 8 one MMA row tile; 9, 10 one tile + 2 DFMA rows; more: two tiles
     const int M = pl->g.numax + 1;
-    if (M <= 8) return launch_t<1, 0, DT>(pl, psi, nbands, coeff, s);
-    if (M <= 10) return launch_t<1, 2, DT>(pl, psi, nbands, coeff, s);
-    return launch_t<2, 0, DT>(pl, psi, nbands, coeff, s);
+    if (M <= 8) return launch_t<1, 0, DT, G>(pl, psi, nbands, coeff, s);
+    if (M <= 10) return launch_t<1, 2, DT, G>(pl, psi, nbands, coeff, s);
+    return launch_t<2, 0, DT, G>(pl, psi, nbands, coeff, s);
+}
+
+template <int DT>
+static sho_status launch_m(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s)
+{
+    // Loads are issued kProjG = 2 steps at a time (longer prefetch distance); a row block with an odd number of
+    // steps then wastes one.  Real data has few, long steps (16 or 32 columns): when more than 6 % of them would
+    // be lost, issue them one by one (cfg 3: 4-5 steps per row block, 1.90 vs 2.03 ms; cfg 4: 8, 15.5 vs 16.1 ms).
+    if (!Elem<DT>::cplx && pl->proj_odd_steps > 0.06) return launch_mg<DT, 1>(pl, psi, nbands, coeff, s);
+    return launch_mg<DT, kProjG>(pl, psi, nbands, coeff, s);
 }
 
 sho_status launch_project(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s)
