@@ -374,6 +374,9 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
                 cp_async(reinterpret_cast<char*>(entw + buf) + 16 * lane,
                          reinterpret_cast<const char*>(p.tile_ent + ci.y + (gs - cbase_s)) + 16 * lane, 16);
         };
+        // K steps per row tile of the z stage, 2 bits each (nks - 1), kept in registers (<= 17 tiles)
+        unsigned long long nks_packed = 0;
+        for (int mt = 0; mt < nmt; ++mt) nks_packed |= (unsigned long long)(p.zt.nks[mt] - 1) << (2 * mt);
         int G = pw;
         bool more = seek(G);
         if (more) fetch_entry(G, 0);
@@ -450,16 +453,19 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
                 const double wr = en->wr, wi = en->wi;
                 const bool phased = !(wr == 1.0 && wi == 0.0);                  // warp-uniform; most images have none
                 double* t2 = T2 + (size_t)slot * T2S + (size_t)(2 * t) * npp;
+                int blk_run = 0;                     // first K block of row tile mt0 (the tiles' blocks are consecutive)
                 for (int mt0 = 0; mt0 < nmt; mt0 += 2) {
                     double d[2][2][2];
                     int nks[2];
 #pragma unroll
                     for (int u = 0; u < 2; ++u) {
-                        nks[u] = (mt0 + u < nmt) ? p.zt.nks[mt0 + u] : 0;
+                        nks[u] = (mt0 + u < nmt) ? (int)((nks_packed >> (2 * (mt0 + u))) & 3) + 1 : 0;
                         d[u][0][0] = d[u][0][1] = d[u][1][0] = d[u][1][1] = 0.0;
                     }
+                    const int blk_u[2] = { blk_run, blk_run + nks[0] };
+                    blk_run += nks[0] + nks[1];
                     auto zstep = [&](int u, int ks, double bzk) {
-                        const real_t* ap = stg + (size_t)((p.zt.blk0[mt0 + u] + ks) * 32 + lane) * 2;
+                        const real_t* ap = stg + (size_t)((blk_u[u] + ks) * 32 + lane) * 2;
                         double a0, a1;
                         load2_rw(ap, a0, a1);
                         if (CPLX && phased) {                                 // conjugate Bloch phase of the image
