@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -54,6 +55,9 @@ static void plan_free_device(sho_plan* p)
     cudaFree(p->d_atoms); cudaFree(p->d_order); cudaFree(p->d_nxyz);
     cudaFree(p->d_tile_ptr); cudaFree(p->d_tile_ent); cudaFree(p->d_tile_list); cudaFree(p->d_tile_info); cudaFree(p->d_cainv); cudaFree(p->d_t2pos); cudaFree(p->d_cidx);
     cudaFree(p->ws_psi); cudaFree(p->ws_c);
+    if (p->s_in) cudaStreamDestroy(p->s_in);
+    if (p->s_out) cudaStreamDestroy(p->s_out);
+    p->s_in = nullptr; p->s_out = nullptr;
     p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr; p->d_cidx = nullptr;
     p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr; p->d_tile_info = nullptr;
     p->ws_psi = nullptr; p->ws_c = nullptr;
@@ -124,6 +128,7 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
     p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr;
     p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr; p->d_tile_info = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr; p->d_cidx = nullptr;
     p->ws_psi = nullptr; p->ws_c = nullptr; p->ws_psi_bytes = 0; p->ws_c_bytes = 0;
+    p->s_in = nullptr; p->s_out = nullptr;
     p->rcut_sigma = rcut_sigma;
     p->dtype = dtype;
     std::memset(&p->g, 0, sizeof(p->g));
@@ -478,23 +483,89 @@ static sho_status ws_reserve(void** ws, size_t* have, size_t need, const char* w
     return SHO_OK;
 }
 
+// The bands are independent, so the host-buffer calls pipeline them in chunks: the H2D copy of chunk i+1, the
+// kernel of chunk i and the D2H copy of chunk i-1 run at the same time on three streams (PCIe is full duplex).
+// A chunk's coefficients [natoms][chunk][N_SHO] are a 2D sub-array of the caller's [natoms][nbands][N_SHO].
+struct HostPipe {
+    cudaStream_t s, s_in, s_out;
+    std::vector<cudaEvent_t> ev;
+    cudaEvent_t event()
+    {
+        cudaEvent_t e = nullptr;
+        cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+        ev.push_back(e);
+        return e;
+    }
+    void after(cudaStream_t waiter, cudaStream_t signaller)      // waiter continues after what signaller has queued
+    {
+        cudaEvent_t e = event();
+        cudaEventRecord(e, signaller);
+        cudaStreamWaitEvent(waiter, e, 0);
+    }
+    ~HostPipe() { for (cudaEvent_t e : ev) cudaEventDestroy(e); }
+};
+
+static sho_status host_pipe_open(sho_plan* plan, cudaStream_t s, HostPipe* hp, const char* what)
+{
+    if (!plan->s_in && cudaStreamCreateWithFlags(&plan->s_in, cudaStreamNonBlocking) != cudaSuccess)
+        return cuda_fail(cudaGetLastError(), what);
+    if (!plan->s_out && cudaStreamCreateWithFlags(&plan->s_out, cudaStreamNonBlocking) != cudaSuccess)
+        return cuda_fail(cudaGetLastError(), what);
+    hp->s = s; hp->s_in = plan->s_in; hp->s_out = plan->s_out;
+    hp->after(hp->s_in, s);                 // the copies start after what the caller queued on its stream
+    hp->after(hp->s_out, s);
+    return SHO_OK;
+}
+
+// bands per chunk: about 512 MB of psi, an even number (the add kernel pairs real bands), at most 16 chunks
+static int host_chunk_bands(const sho_plan* plan, int nbands)
+{
+    if (const char* env = std::getenv("SHO_HOST_CHUNK_BANDS")) {            // tuning / test knob
+        const int v = std::atoi(env);
+        if (v > 0) return std::min(v, nbands);
+    }
+    const double band_bytes = (double)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * elem_size(plan->dtype);
+    int cb = (int)std::max(1.0, std::floor(512.0e6 / band_bytes));
+    cb = std::max(cb, (nbands + 15) / 16);
+    if (cb > 1) cb += cb & 1;
+    return std::min(cb, nbands);
+}
+
 sho_status sho_project_host(sho_plan* plan, const void* psi_host, int32_t nbands, void* coeff_host, void* cuda_stream)
 {
     sho_status st = check_hot("sho_project_host", plan, psi_host, coeff_host, nbands);
     if (st != SHO_OK) return st;
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     const size_t esz = elem_size(plan->dtype);
-    const size_t psi_bytes = (size_t)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * nbands * esz;
-    const size_t c_bytes = (size_t)plan->g.natoms * nbands * plan->g.nsho * esz;
-    if ((st = ws_reserve(&plan->ws_psi, &plan->ws_psi_bytes, psi_bytes, "sho_project_host")) != SHO_OK) return st;
+    const size_t band_bytes = (size_t)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * esz;
+    const size_t row_bytes = (size_t)plan->g.nsho * esz;                     // coefficients of one (atom, band)
+    const size_t c_bytes = (size_t)plan->g.natoms * nbands * row_bytes;
+    if ((st = ws_reserve(&plan->ws_psi, &plan->ws_psi_bytes, band_bytes * nbands, "sho_project_host")) != SHO_OK) return st;
     if ((st = ws_reserve(&plan->ws_c, &plan->ws_c_bytes, std::max<size_t>(c_bytes, 16), "sho_project_host")) != SHO_OK) return st;
-    cudaError_t e = cudaMemcpyAsync(plan->ws_psi, psi_host, psi_bytes, cudaMemcpyHostToDevice, s);
-    if (e != cudaSuccess) return cuda_fail(e, "sho_project_host: H2D psi");
-    if (plan->g.natoms > 0) {
-        if ((st = launch_project(plan, plan->ws_psi, nbands, plan->ws_c, s)) != SHO_OK) return st;
-        e = cudaMemcpyAsync(coeff_host, plan->ws_c, c_bytes, cudaMemcpyDeviceToHost, s);
-        if (e != cudaSuccess) return cuda_fail(e, "sho_project_host: D2H coeff");
+    HostPipe hp;
+    if ((st = host_pipe_open(plan, s, &hp, "sho_project_host: streams")) != SHO_OK) return st;
+    const int cb = host_chunk_bands(plan, nbands);
+    cudaError_t e = cudaSuccess;
+    size_t c_off = 0;
+    for (int b0 = 0; b0 < nbands; b0 += cb) {
+        const int nb = std::min(cb, nbands - b0);
+        char* d_psi = static_cast<char*>(plan->ws_psi) + (size_t)b0 * band_bytes;
+        char* d_c = static_cast<char*>(plan->ws_c) + c_off;                   // [natoms][nb][N_SHO]
+        e = cudaMemcpyAsync(d_psi, static_cast<const char*>(psi_host) + (size_t)b0 * band_bytes, band_bytes * nb,
+                            cudaMemcpyHostToDevice, hp.s_in);
+        if (e != cudaSuccess) return cuda_fail(e, "sho_project_host: H2D psi");
+        hp.after(s, hp.s_in);
+        if (plan->g.natoms > 0) {
+            if ((st = launch_project(plan, d_psi, nb, d_c, s)) != SHO_OK) return st;
+            hp.after(hp.s_out, s);
+            e = cudaMemcpy2DAsync(static_cast<char*>(coeff_host) + (size_t)b0 * row_bytes, (size_t)nbands * row_bytes, d_c,
+                                  (size_t)nb * row_bytes, (size_t)nb * row_bytes, (size_t)plan->g.natoms,
+                                  cudaMemcpyDeviceToHost, hp.s_out);
+            if (e != cudaSuccess) return cuda_fail(e, "sho_project_host: D2H coeff");
+        }
+        c_off += (size_t)plan->g.natoms * nb * row_bytes;
     }
+    hp.after(s, hp.s_out);
     e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return cuda_fail(e, "sho_project_host: synchronize");
     return SHO_OK;
@@ -506,18 +577,37 @@ sho_status sho_add_host(sho_plan* plan, const void* coeff_host, int32_t nbands, 
     if (st != SHO_OK) return st;
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     const size_t esz = elem_size(plan->dtype);
-    const size_t psi_bytes = (size_t)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * nbands * esz;
-    const size_t c_bytes = (size_t)plan->g.natoms * nbands * plan->g.nsho * esz;
+    const size_t band_bytes = (size_t)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * esz;
+    const size_t row_bytes = (size_t)plan->g.nsho * esz;
+    const size_t c_bytes = (size_t)plan->g.natoms * nbands * row_bytes;
     if (plan->g.natoms == 0 || plan->n_tile_list == 0) return SHO_OK;
-    if ((st = ws_reserve(&plan->ws_psi, &plan->ws_psi_bytes, psi_bytes, "sho_add_host")) != SHO_OK) return st;
+    if ((st = ws_reserve(&plan->ws_psi, &plan->ws_psi_bytes, band_bytes * nbands, "sho_add_host")) != SHO_OK) return st;
     if ((st = ws_reserve(&plan->ws_c, &plan->ws_c_bytes, std::max<size_t>(c_bytes, 16), "sho_add_host")) != SHO_OK) return st;
-    cudaError_t e = cudaMemcpyAsync(plan->ws_psi, psi_host, psi_bytes, cudaMemcpyHostToDevice, s);
-    if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: H2D psi");
-    e = cudaMemcpyAsync(plan->ws_c, coeff_host, c_bytes, cudaMemcpyHostToDevice, s);
-    if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: H2D coeff");
-    if ((st = launch_add(plan, plan->ws_c, nbands, plan->ws_psi, s)) != SHO_OK) return st;
-    e = cudaMemcpyAsync(psi_host, plan->ws_psi, psi_bytes, cudaMemcpyDeviceToHost, s);
-    if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: D2H psi");
+    HostPipe hp;
+    if ((st = host_pipe_open(plan, s, &hp, "sho_add_host: streams")) != SHO_OK) return st;
+    const int cb = host_chunk_bands(plan, nbands);
+    cudaError_t e = cudaSuccess;
+    size_t c_off = 0;
+    for (int b0 = 0; b0 < nbands; b0 += cb) {
+        const int nb = std::min(cb, nbands - b0);
+        char* d_psi = static_cast<char*>(plan->ws_psi) + (size_t)b0 * band_bytes;
+        char* d_c = static_cast<char*>(plan->ws_c) + c_off;                   // [natoms][nb][N_SHO]
+        e = cudaMemcpy2DAsync(d_c, (size_t)nb * row_bytes, static_cast<const char*>(coeff_host) + (size_t)b0 * row_bytes,
+                              (size_t)nbands * row_bytes, (size_t)nb * row_bytes, (size_t)plan->g.natoms,
+                              cudaMemcpyHostToDevice, hp.s_in);
+        if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: H2D coeff");
+        e = cudaMemcpyAsync(d_psi, static_cast<const char*>(psi_host) + (size_t)b0 * band_bytes, band_bytes * nb,
+                            cudaMemcpyHostToDevice, hp.s_in);
+        if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: H2D psi");
+        hp.after(s, hp.s_in);
+        if ((st = launch_add(plan, d_c, nb, d_psi, s)) != SHO_OK) return st;
+        hp.after(hp.s_out, s);
+        e = cudaMemcpyAsync(static_cast<char*>(psi_host) + (size_t)b0 * band_bytes, d_psi, band_bytes * nb,
+                            cudaMemcpyDeviceToHost, hp.s_out);
+        if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: D2H psi");
+        c_off += (size_t)plan->g.natoms * nb * row_bytes;
+    }
+    hp.after(s, hp.s_out);
     e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: synchronize");
     return SHO_OK;

@@ -99,6 +99,7 @@ struct sho_plan {
     // workspace for the *_host calls
     void* ws_psi; size_t ws_psi_bytes;
     void* ws_c;   size_t ws_c_bytes;
+    cudaStream_t s_in, s_out;              // copy streams of the *_host calls (created on first use)
 };
 
 struct sho_tables {

@@ -357,6 +357,27 @@ def test_host_buffer_entry_points(sho):
     plan.close()
 
 
+@pytest.mark.parametrize("k,chunk", [(3, "2"), (3, "3"), (5, "1"), (5, "2")])
+def test_host_buffer_calls_pipeline_band_chunks(sho, k, chunk, monkeypatch):
+    # the *_host calls copy and compute band chunks on three streams; force several (ragged) chunks
+    monkeypatch.setenv("SHO_HOST_CHUNK_BANDS", chunk)
+    w = workloads.make(k, size="small")
+    wide = np.complex128 if w.is_complex else np.float64
+    plan = sho.plan_for(w)
+    try:
+        psi = w.psi()
+        c = np.zeros((w.natoms, w.nbands, plan.nsho), dtype=psi.dtype)
+        plan.project_host(psi, c)
+        check_project(sho, w, psi, c, TOL[w.dtype])
+        coeff = w.coeff(plan.nsho)
+        out = psi.copy()
+        plan.add_host(coeff, out)
+        ref = oracle.add(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax, coeff.astype(wide), psi.astype(wide))
+        assert np.abs(out - ref).max() <= TOL[w.dtype] * np.abs(ref).max()
+    finally:
+        plan.close()
+
+
 def test_wrong_arguments_raise(sho):
     import torch
     w = workloads.make(1)
