@@ -131,6 +131,42 @@ __device__ __forceinline__ void cp_async(void* smem_dst, const void* gmem_src, i
     else asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;\n" ::"r"(d), "l"(gmem_src), "r"(n) : "memory");
 }
 
+// z stage of two row tiles (N0 >= N1 K steps; N1 = 0: one tile) as straight-line code: every operand is
+// loaded first, the MMAs of the two tiles and the two channels alternate (four accumulator chains)
+template <int N0, int N1, bool CPLX, typename real_t>
+__device__ __forceinline__ void add_zpair(const real_t* __restrict__ a0p, const real_t* __restrict__ a1p,
+                                          const double* __restrict__ fz, bool phased, double wr, double wi,
+                                          double (&d)[2][2][2])
+{
+    double bz[N0], a[2][N0][2];
+#pragma unroll
+    for (int ks = 0; ks < N0; ++ks) {
+        bz[ks] = fz[ks * 32];                                                    // B[k = nz][col = plane]
+        load2_rw(a0p + ks * 64, a[0][ks][0], a[0][ks][1]);
+        if (ks < N1) load2_rw(a1p + ks * 64, a[1][ks][0], a[1][ks][1]);
+    }
+    if (CPLX && phased) {                                                        // conjugate Bloch phase of the image
+#pragma unroll
+        for (int ks = 0; ks < N0; ++ks)
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+                if (u == 0 || ks < N1) {
+                    const double re = a[u][ks][0], im = a[u][ks][1];
+                    a[u][ks][0] = re * wr - im * wi;
+                    a[u][ks][1] = re * wi + im * wr;
+                }
+    }
+#pragma unroll
+    for (int ks = 0; ks < N0; ++ks) {
+        dmma(d[0][0][0], d[0][0][1], a[0][ks][0], bz[ks]);
+        dmma(d[0][1][0], d[0][1][1], a[0][ks][1], bz[ks]);
+        if (ks < N1) {
+            dmma(d[1][0][0], d[1][0][1], a[1][ks][0], bz[ks]);
+            dmma(d[1][1][0], d[1][1][1], a[1][ks][1], bz[ks]);
+        }
+    }
+}
+
 template <int KQ, int DT>
 __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_constant__ AddParams p)
 {
@@ -499,29 +535,20 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
                     }
                     const int blk_u[2] = { blk_run, blk_run + nks[0] };
                     blk_run += nks[0] + nks[1];
-                    auto zstep = [&](int u, int ks, double bzk) {
-                        const real_t* ap = stg + (size_t)((blk_u[u] + ks) * 32 + lane) * 2;
-                        double a0, a1;
-                        load2_rw(ap, a0, a1);
-                        if (CPLX && phased) {                                 // conjugate Bloch phase of the image
-                            const double re = a0, im = a1;
-                            a0 = re * wr - im * wi;
-                            a1 = re * wi + im * wr;
-                        }
-                        dmma(d[u][0][0], d[u][0][1], a0, bzk);
-                        dmma(d[u][1][0], d[u][1][1], a1, bzk);
-                    };
-                    // the tiles are sorted by ny+nx, so nks[0] >= nks[1]: K steps of both, then of the first alone,
-                    // in loops with run-time bounds (real branches: a predicated-off DMMA still costs its pipe time)
-                    int ks = 0;
-#pragma unroll 1
-                    for (; ks < nks[1]; ++ks) {
-                        const double bzk = fzw[ks * 32 + lane];                  // B[k = nz][col = plane]
-                        zstep(0, ks, bzk);
-                        zstep(1, ks, bzk);
+                    // one straight-line variant per (K steps of the first tile, of the second): entered by a jump,
+                    // so no MMA is predicated (a predicated-off DMMA still costs its pipe time)
+                    const real_t* a0p = stg + (size_t)(blk_u[0] * 32 + lane) * 2;
+                    const real_t* a1p = stg + (size_t)(blk_u[1] * 32 + lane) * 2;
+                    const double* fzl = fzw + lane;
+#define SHO_ZCASE(N0, N1) case (N0) * 8 + (N1): if constexpr ((N0) <= KQ) add_zpair<N0, N1, CPLX>(a0p, a1p, fzl, phased, wr, wi, d); break;
+                    switch (nks[0] * 8 + nks[1]) {
+                        SHO_ZCASE(1, 0) SHO_ZCASE(1, 1)
+                        SHO_ZCASE(2, 0) SHO_ZCASE(2, 1) SHO_ZCASE(2, 2)
+                        SHO_ZCASE(3, 0) SHO_ZCASE(3, 1) SHO_ZCASE(3, 2) SHO_ZCASE(3, 3)
+                        SHO_ZCASE(4, 0) SHO_ZCASE(4, 1) SHO_ZCASE(4, 2) SHO_ZCASE(4, 3) SHO_ZCASE(4, 4)
+                        default: break;
                     }
-#pragma unroll 1
-                    for (; ks < nks[0]; ++ks) zstep(0, ks, fzw[ks * 32 + lane]);
+#undef SHO_ZCASE
 #pragma unroll
                     for (int u = 0; u < 2; ++u)
                         if (nks[u] > 0) {
