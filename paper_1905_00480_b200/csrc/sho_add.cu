@@ -249,7 +249,6 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
 #pragma unroll
             for (int ks = 0; ks < KQ; ++ks) t2off[nt][ks] = p.t2pos[16 * (8 * nt + 4 * (q & 1) + (q >> 1)) + 4 * ks + t];
 
-        const bool rem89 = p.g.numax <= 9;                 // (KQ == 3) the third K step holds only ny = 8, 9
         int slot = 0, ph = 0;
         const double* fxy = FXY + lane;
         const double* t2p = T2 + (size_t)(ch * kAddTZ + plane) * npp;
@@ -300,52 +299,18 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
         _Pragma("unroll") for (int kk = 0; kk < KQ; ++kk) a_[kk] = fxy[((YT) * KQ + kk) * 32];          \
         _Pragma("unroll") for (int kk = 0; kk < KQ; ++kk) dmma(D[YT][0], D[YT][1], a_[kk], D1[kk >> 1][kk & 1]); \
     }
-                    // numax = 8, 9: the third K step holds only ny = 8, 9.  Two DFMAs per output replace its MMA
-                    // (half the pipe time): T1[x][8], T1[x][9] of this lane's two columns come from the lanes that
-                    // hold them in the x-stage fragment, phi_8(y), phi_9(y) of its row from the table.
-#define SHO_ADD_YBLOCK_R(YT)                                                                            \
-    {                                                                                                   \
-        const double a0_ = fxy[((YT) * KQ) * 32], a1_ = fxy[((YT) * KQ + 1) * 32];                      \
-        const double2 f_ = *reinterpret_cast<const double2*>(fq + ((YT) * KQ + 2) * 32);                \
-        D[YT][0] = fma(f_.x, t8[0], fma(f_.y, t9[0], D[YT][0]));                                        \
-        D[YT][1] = fma(f_.x, t8[1], fma(f_.y, t9[1], D[YT][1]));                                        \
-        dmma(D[YT][0], D[YT][1], a0_, D1[0][0]);                                                        \
-        dmma(D[YT][0], D[YT][1], a1_, D1[0][1]);                                                        \
-    }
-                    if (KQ == 3 && rem89) {
-                        double t8[2], t9[2];
-#pragma unroll
-                        for (int sx = 0; sx < 2; ++sx) {
-                            t8[sx] = __shfl_sync(0xffffffffu, D1[NT - 1][0], 4 * (2 * t + sx));
-                            t9[sx] = __shfl_sync(0xffffffffu, D1[NT - 1][0], 4 * (2 * t + sx) + 1);
-                        }
-                        const double* fq = fxy - lane + q * 4;
-                        switch (ytlo) {
-                            case 0: SHO_ADD_YBLOCK_R(0) if (ythi == 0) break;
-                            case 1: SHO_ADD_YBLOCK_R(1) if (ythi == 1) break;
-                            case 2: SHO_ADD_YBLOCK_R(2) if (ythi == 2) break;
-                            case 3: SHO_ADD_YBLOCK_R(3) if (ythi == 3) break;
-                            case 4: SHO_ADD_YBLOCK_R(4) if (ythi == 4) break;
-                            case 5: SHO_ADD_YBLOCK_R(5) if (ythi == 5) break;
-                            case 6: SHO_ADD_YBLOCK_R(6) if (ythi == 6) break;
-                            case 7: SHO_ADD_YBLOCK_R(7)
-                            default: break;
-                        }
-                    } else {
-                        switch (ytlo) {
-                            case 0: SHO_ADD_YBLOCK(0) if (ythi == 0) break;
-                            case 1: SHO_ADD_YBLOCK(1) if (ythi == 1) break;
-                            case 2: SHO_ADD_YBLOCK(2) if (ythi == 2) break;
-                            case 3: SHO_ADD_YBLOCK(3) if (ythi == 3) break;
-                            case 4: SHO_ADD_YBLOCK(4) if (ythi == 4) break;
-                            case 5: SHO_ADD_YBLOCK(5) if (ythi == 5) break;
-                            case 6: SHO_ADD_YBLOCK(6) if (ythi == 6) break;
-                            case 7: SHO_ADD_YBLOCK(7)
-                            default: break;
-                        }
+                    switch (ytlo) {
+                        case 0: SHO_ADD_YBLOCK(0) if (ythi == 0) break;
+                        case 1: SHO_ADD_YBLOCK(1) if (ythi == 1) break;
+                        case 2: SHO_ADD_YBLOCK(2) if (ythi == 2) break;
+                        case 3: SHO_ADD_YBLOCK(3) if (ythi == 3) break;
+                        case 4: SHO_ADD_YBLOCK(4) if (ythi == 4) break;
+                        case 5: SHO_ADD_YBLOCK(5) if (ythi == 5) break;
+                        case 6: SHO_ADD_YBLOCK(6) if (ythi == 6) break;
+                        case 7: SHO_ADD_YBLOCK(7)
+                        default: break;
                     }
 #undef SHO_ADD_YBLOCK
-#undef SHO_ADD_YBLOCK_R
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(empty + slot);
