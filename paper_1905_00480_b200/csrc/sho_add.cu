@@ -31,7 +31,7 @@
 
 namespace sho {
 
-constexpr int kAddXYWarps = 2 * kAddTZ;     // (plane, channel)
+constexpr int kAddXYWarps = 2 * kAddTZ;     // (plane, half of the rows)
 constexpr int kAddPWarps = 8;               // producer warps, one pair each at a time
 constexpr int kAddThreads = (kAddXYWarps + kAddPWarps) * 32;
 
@@ -58,7 +58,7 @@ struct AddParams {
 };
 
 // shared-memory carve-up (doubles): [FXY: RD x 9 KQ 32][T2: RD x 2 x 8 npp][FZ: npw x KQ 32][STG: npw x stg]
-// [EXPT: 64][XCH: complex write-back exchange][ENT: npw x 2 records] then [META: RD int32][ZPOS: 8 nmt uint16][CIDX: 32 nblk uint16][mbarriers: full RD, empty RD]
+// [EXPT: 64][ENT: npw x 2 records] then [META: RD int32][ZPOS: 8 nmt uint16][CIDX: 32 nblk uint16][mbarriers: full RD, empty RD]
 template <int KQ>
 struct AddSmem {
     static constexpr int FXYS = 9 * KQ * 32;
@@ -69,8 +69,7 @@ struct AddSmem {
     static __host__ __device__ size_t bytes(int rd, int npw, int nmt, int nblk, int real_bytes, bool cplx)
     {
         const int npp = 8 * nmt + 2;
-        size_t b = 8 * ((size_t)rd * (FXYS + t2s(npp)) + (size_t)npw * (FZS + stg(nblk, real_bytes)) + 64 +
-                        (cplx ? (size_t)kAddTZ * kAddTY * kAddTX : 0));
+        size_t b = 8 * ((size_t)rd * (FXYS + t2s(npp)) + (size_t)npw * (FZS + stg(nblk, real_bytes)) + 64);
         b += (size_t)npw * 2 * sizeof(AddEntry);
         b += (size_t)rd * 4 + (size_t)8 * nmt * 2 + (size_t)32 * nblk * 2;
         b = (b + 7) & ~(size_t)7;
@@ -195,8 +194,7 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
     double* FZ = T2 + (size_t)RD * T2S;                   // [npw][KQ][32]
     double* STG = FZ + (size_t)NPW * FZS;                 // [npw][STGS]   z-stage A fragments of the pair in production, element type of the data
     double* EXPT = STG + (size_t)NPW * STGS;              // [64]  2^(j/64), see exp_neg
-    double* XCH = EXPT + 64;                              // complex only: [8 planes][64 x 8] imaginary parts on their way out
-    AddEntry* ENTW = reinterpret_cast<AddEntry*>(XCH + (CPLX ? kAddTZ * kAddTY * kAddTX : 0));                     // [npw][2]  this and the next record
+    AddEntry* ENTW = reinterpret_cast<AddEntry*>(EXPT + 64);                     // [npw][2]  this and the next record
     int32_t* META = reinterpret_cast<int32_t*>(ENTW + 2 * NPW);                  // [RD] zmask | ytlo << 8 | ythi << 16
     uint16_t* ZPOS = reinterpret_cast<uint16_t*>(META + RD);                     // [8 nmt] T2 column of z-stage row
     uint16_t* CIDX = ZPOS + 8 * nmt;                                             // [nblk][32] coefficient of an A-fragment element
@@ -239,6 +237,139 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
     __syncthreads();
 
     if (warp < kAddXYWarps) {
+      // Two mappings of the 16 XY warps (measured): complex data -- boxes of about one tile height at the configs --
+      // run (plane, half of the rows) with both channels per warp; real data runs (plane, channel).
+      if constexpr (CPLX) {
+        // =============================== XY warps ===============================
+        // warp = (z plane, half of the 64 rows): four 8-row blocks of BOTH channels, so that one A-fragment load
+        // feeds two MMAs and two accumulator chains alternate; the write-back needs no exchange
+        const int plane = warp & 7, half = warp >> 3;
+        // x stage, B fragment B[k = nx][col = ny]: this lane reads T2[(ny,nx)] with nx = 4 ks + t and
+        // ny = 8 nt + 4 (q & 1) + (q >> 1); pairs outside the basis read the zero column
+        int t2off[NT][KQ];
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+            for (int ks = 0; ks < KQ; ++ks) t2off[nt][ks] = p.t2pos[16 * (8 * nt + 4 * (q & 1) + (q >> 1)) + 4 * ks + t];
+
+        int slot = 0, ph = 0;
+        const double* fxy = FXY + lane;
+        const double* t2p = T2 + (size_t)plane * npp;                       // channel 1: + kAddTZ * npp
+        int4 info_next = item_info(blockIdx.x);
+        for (int item = blockIdx.x; item < p.nitems; item += gridDim.x) {
+            const Item it = decode(info_next);
+            if (item + (int)gridDim.x < p.nitems) info_next = item_info(item + gridDim.x);   // arrives during this item
+            const int npairs = it.npairs;
+            const bool two = CPLX || (it.b0 + 1 < p.nbands);                // second channel exists
+            const int jz = it.jz0 + plane;
+            const int row0 = it.jy0 + 32 * half;                            // first of this warp's rows
+            real_t* pb = reinterpret_cast<real_t*>(p.psi) + ((size_t)it.b0 * p.band_stride + (size_t)jz * Ny * Nx) * P;
+            // the owned rows are read once, at the end of the item: ask L2 for their lines now
+            if (jz < Nz) {
+                constexpr int kLineElems = 128 / (int)(sizeof(real_t) * P);           // tile columns per 128-byte line
+                for (int r = lane; r < 32 * ((kAddTX + kLineElems - 1) / kLineElems); r += 32) {
+                    const int row = r % 32, seg = r / 32;
+                    if (row0 + row < Ny && it.jx0 + seg * kLineElems < Nx) {
+                        const real_t* a = pb + ((size_t)(row0 + row) * Nx + it.jx0 + seg * kLineElems) * P;
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+                        if (!CPLX && two) asm volatile("prefetch.global.L2 [%0];" ::"l"(a + p.band_stride));
+                    }
+                }
+            }
+            double D[4][2][2];                                              // [block][channel][column]
+#pragma unroll
+            for (int yt = 0; yt < 4; ++yt) D[yt][0][0] = D[yt][0][1] = D[yt][1][0] = D[yt][1][1] = 0.0;
+
+            for (int g = 0; g < npairs; ++g) {
+                mbar_wait(full + slot, ph);
+                const int meta = META[slot];
+                // this warp's share of the touched 8-row blocks ytlo..ythi
+                const int ytlo = max((meta >> 8) & 0xff, 4 * half), ythi = min((meta >> 16) & 0xff, 4 * half + 3);
+                if (((meta >> plane) & 1) && ytlo <= ythi) {
+                    double D1[NT][2][2];
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) D1[nt][0][0] = D1[nt][0][1] = D1[nt][1][0] = D1[nt][1][1] = 0.0;
+#pragma unroll
+                    for (int ks = 0; ks < KQ; ++ks)
+#pragma unroll
+                        for (int nt = 0; nt < NT; ++nt)
+                            if (8 * nt + 4 * ks <= 4 * KQ - 4) {            // the block holds some ny+nx <= numax (numax >= 4 KQ - 4)
+                                const double a = fxy[(8 * KQ + ks) * 32];
+                                dmma(D1[nt][0][0], D1[nt][0][1], a, t2p[t2off[nt][ks]]);
+                                dmma(D1[nt][1][0], D1[nt][1][1], a, t2p[(size_t)kAddTZ * npp + t2off[nt][ks]]);
+                            }
+                    // A predicated-off DMMA still takes its 16 cycles of the pipe (measured), and the compiler
+                    // predicates a short "if": enter the unrolled blocks by a jump (eight cases make a jump table;
+                    // a warp only ever uses its four) and leave them by a branch instead.
+#define SHO_ADD_YBLOCK(YT)                                                                              \
+    {                                                                                                   \
+        double a_[KQ];                                                                                  \
+        _Pragma("unroll") for (int kk = 0; kk < KQ; ++kk) a_[kk] = fxy[((YT) * KQ + kk) * 32];          \
+        _Pragma("unroll") for (int kk = 0; kk < KQ; ++kk) {                                             \
+            dmma(D[(YT) & 3][0][0], D[(YT) & 3][0][1], a_[kk], D1[kk >> 1][0][kk & 1]);                 \
+            dmma(D[(YT) & 3][1][0], D[(YT) & 3][1][1], a_[kk], D1[kk >> 1][1][kk & 1]);                 \
+        }                                                                                               \
+    }
+                    switch (ytlo) {
+                        case 0: SHO_ADD_YBLOCK(0) if (ythi == 0) break;
+                        case 1: SHO_ADD_YBLOCK(1) if (ythi == 1) break;
+                        case 2: SHO_ADD_YBLOCK(2) if (ythi == 2) break;
+                        case 3: SHO_ADD_YBLOCK(3) break;
+                        case 4: SHO_ADD_YBLOCK(4) if (ythi == 4) break;
+                        case 5: SHO_ADD_YBLOCK(5) if (ythi == 5) break;
+                        case 6: SHO_ADD_YBLOCK(6) if (ythi == 6) break;
+                        case 7: SHO_ADD_YBLOCK(7)
+                        default: break;
+                    }
+#undef SHO_ADD_YBLOCK
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + slot);
+                fxy += FXYS; t2p += T2S;
+                if (++slot == RD) { slot = 0; ph ^= 1; fxy = FXY + lane; t2p = T2 + (size_t)plane * npp; }
+            }
+
+            // ---------------- one read-modify-write of the owned rows ----------------
+            if (jz < Nz) {
+                const int jx = it.jx0 + 2 * t;
+#pragma unroll
+                for (int yt = 0; yt < 4; ++yt) {
+                    const int jy = row0 + 8 * yt + q;
+                    if (jy < Ny && jx < Nx) {
+                        if (CPLX) {
+                            real_t* pc = pb + ((size_t)jy * Nx + jx) * 2;
+#pragma unroll
+                            for (int sx = 0; sx < 2; ++sx)
+                                if (jx + sx < Nx) {
+                                    if (p.vec_ok) {
+                                        double v0, v1;
+                                        load2_rw(pc + 2 * sx, v0, v1);
+                                        store2(pc + 2 * sx, v0 + D[yt][0][sx], v1 + D[yt][1][sx]);
+                                    } else {
+                                        pc[2 * sx] = (real_t)((double)pc[2 * sx] + D[yt][0][sx]);
+                                        pc[2 * sx + 1] = (real_t)((double)pc[2 * sx + 1] + D[yt][1][sx]);
+                                    }
+                                }
+                        } else {
+#pragma unroll
+                            for (int c = 0; c < 2; ++c)
+                                if (c == 0 || two) {
+                                    real_t* pp_ = pb + (size_t)c * p.band_stride + ((size_t)jy * Nx + jx);
+                                    if (p.vec_ok && jx + 1 < Nx) {
+                                        double v0, v1;
+                                        load2_rw(pp_, v0, v1);
+                                        store2(pp_, v0 + D[yt][c][0], v1 + D[yt][c][1]);
+                                    } else {
+                                        pp_[0] = (real_t)((double)pp_[0] + D[yt][c][0]);
+                                        if (jx + 1 < Nx) pp_[1] = (real_t)((double)pp_[1] + D[yt][c][1]);
+                                    }
+                                }
+                        }
+                    }
+                }
+            }
+        }
+      } else {
         // =============================== XY warps ===============================
         const int plane = warp & 7, ch = warp >> 3;
         // x stage, B fragment B[k = nx][col = ny]: this lane reads T2[(ny,nx)] with nx = 4 ks + t and
@@ -319,44 +450,7 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
             }
 
             // ---------------- one read-modify-write of the owned rows ----------------
-            if (CPLX) {
-                // the warp of the imaginary part hands its accumulators to the warp of the real part through
-                // shared memory, so that psi is read and written as whole complex numbers
-                double* xch = XCH + (size_t)plane * (kAddTY * kAddTX);
-                if (ch == 1) {
-#pragma unroll
-                    for (int yt = 0; yt < NYT; ++yt) {
-                        double2 v; v.x = D[yt][0]; v.y = D[yt][1];
-                        *reinterpret_cast<double2*>(xch + (8 * yt + q) * kAddTX + 2 * t) = v;
-                    }
-                }
-                asm volatile("bar.sync 1, %0;\n" ::"r"(kAddXYWarps * 32) : "memory");
-                if (ch == 0 && jz < Nz) {
-                    const int jx = it.jx0 + 2 * t;
-#pragma unroll
-                    for (int yt = 0; yt < NYT; ++yt) {
-                        const int jy = it.jy0 + 8 * yt + q;
-                        const double2 im = *reinterpret_cast<const double2*>(xch + (8 * yt + q) * kAddTX + 2 * t);
-                        if (jy < Ny) {
-                            real_t* pc = pb + ((size_t)jy * Nx + jx) * 2;
-#pragma unroll
-                            for (int sx = 0; sx < 2; ++sx)
-                                if (jx + sx < Nx) {
-                                    const double dre = D[yt][sx], dim = sx ? im.y : im.x;
-                                    if (p.vec_ok) {
-                                        double v0, v1;
-                                        load2_rw(pc + 2 * sx, v0, v1);
-                                        store2(pc + 2 * sx, v0 + dre, v1 + dim);
-                                    } else {
-                                        pc[2 * sx] = (real_t)((double)pc[2 * sx] + dre);
-                                        pc[2 * sx + 1] = (real_t)((double)pc[2 * sx + 1] + dim);
-                                    }
-                                }
-                        }
-                    }
-                }
-                asm volatile("bar.sync 1, %0;\n" ::"r"(kAddXYWarps * 32) : "memory");     // the exchange buffer is free again
-            } else if (active && jz < Nz) {
+            if (active && jz < Nz) {
                 const int jx = it.jx0 + 2 * t;
 #pragma unroll
                 for (int yt = 0; yt < NYT; ++yt) {
@@ -375,6 +469,7 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
                 }
             }
         }
+      }
     } else {
         // =============================== producer warps ===============================
         // Warp pw produces pairs pw, pw + NPW, ... on its own: tables, coefficients, z stage.  Its latency per
