@@ -31,9 +31,10 @@
 
 namespace sho {
 
-constexpr int kAddXYWarps = 2 * kAddTZ;     // (plane, half of the rows)
 constexpr int kAddPWarps = 8;               // producer warps, one pair each at a time
-constexpr int kAddThreads = (kAddXYWarps + kAddPWarps) * 32;
+// XY warps: complex data 8 (one z plane, both channels each), real data 16 ((plane, channel))
+__host__ __device__ constexpr int add_xy_warps(bool cplx) { return cplx ? kAddTZ : 2 * kAddTZ; }
+__host__ __device__ constexpr int add_threads(bool cplx) { return (add_xy_warps(cplx) + kAddPWarps) * 32; }
 
 struct AddParams {
     GridDev g;
@@ -167,7 +168,7 @@ __device__ __forceinline__ void add_zpair(const real_t* __restrict__ a0p, const 
 }
 
 template <int KQ, int DT>
-__global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_constant__ AddParams p)
+__global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel(const __grid_constant__ AddParams p)
 {
     using E = Elem<DT>;
     using real_t = typename E::real_t;
@@ -180,6 +181,7 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
     constexpr int FXYS = S::FXYS, FZS = S::FZS;
     constexpr int MTC = (KQ <= 2) ? 4 : 3;     // z-stage row tiles whose coefficients a producer lane holds at once
     static_assert(kAddTX == 8 && kAddTZ == 8, "one 8x8 MMA block per x / z extent");
+    constexpr int kAddXYWarps = add_xy_warps(CPLX), kAddThreads = add_threads(CPLX);
 
     extern __shared__ __align__(16) double smem[];
     const int nsho = p.g.nsho;
@@ -237,13 +239,13 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
     __syncthreads();
 
     if (warp < kAddXYWarps) {
-      // Two mappings of the 16 XY warps (measured): complex data -- boxes of about one tile height at the configs --
-      // run (plane, half of the rows) with both channels per warp; real data runs (plane, channel).
+      // Two mappings of the XY warps (measured): complex data runs 8 warps, one z plane of both channels each (64
+      // accumulator registers, 128 registers per thread); real data runs 16 warps, (plane, channel).
       if constexpr (CPLX) {
         // =============================== XY warps ===============================
-        // warp = (z plane, half of the 64 rows): four 8-row blocks of BOTH channels, so that one A-fragment load
-        // feeds two MMAs and two accumulator chains alternate; the write-back needs no exchange
-        const int plane = warp & 7, half = warp >> 3;
+        // warp = z plane: its 64 rows x 8 columns of BOTH channels (64 accumulator registers), so that one
+        // A-fragment load feeds two MMAs, two accumulator chains alternate and the write-back needs no exchange
+        const int plane = warp;
         // x stage, B fragment B[k = nx][col = ny]: this lane reads T2[(ny,nx)] with nx = 4 ks + t and
         // ny = 8 nt + 4 (q & 1) + (q >> 1); pairs outside the basis read the zero column
         int t2off[NT][KQ];
@@ -262,13 +264,13 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
             const int npairs = it.npairs;
             const bool two = CPLX || (it.b0 + 1 < p.nbands);                // second channel exists
             const int jz = it.jz0 + plane;
-            const int row0 = it.jy0 + 32 * half;                            // first of this warp's rows
+            const int row0 = it.jy0;
             real_t* pb = reinterpret_cast<real_t*>(p.psi) + ((size_t)it.b0 * p.band_stride + (size_t)jz * Ny * Nx) * P;
             // the owned rows are read once, at the end of the item: ask L2 for their lines now
             if (jz < Nz) {
                 constexpr int kLineElems = 128 / (int)(sizeof(real_t) * P);           // tile columns per 128-byte line
-                for (int r = lane; r < 32 * ((kAddTX + kLineElems - 1) / kLineElems); r += 32) {
-                    const int row = r % 32, seg = r / 32;
+                for (int r = lane; r < kAddTY * ((kAddTX + kLineElems - 1) / kLineElems); r += 32) {
+                    const int row = r % kAddTY, seg = r / kAddTY;
                     if (row0 + row < Ny && it.jx0 + seg * kLineElems < Nx) {
                         const real_t* a = pb + ((size_t)(row0 + row) * Nx + it.jx0 + seg * kLineElems) * P;
                         asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
@@ -276,16 +278,15 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
                     }
                 }
             }
-            double D[4][2][2];                                              // [block][channel][column]
+            double D[NYT][2][2];                                            // [block][channel][column]
 #pragma unroll
-            for (int yt = 0; yt < 4; ++yt) D[yt][0][0] = D[yt][0][1] = D[yt][1][0] = D[yt][1][1] = 0.0;
+            for (int yt = 0; yt < NYT; ++yt) D[yt][0][0] = D[yt][0][1] = D[yt][1][0] = D[yt][1][1] = 0.0;
 
             for (int g = 0; g < npairs; ++g) {
                 mbar_wait(full + slot, ph);
                 const int meta = META[slot];
-                // this warp's share of the touched 8-row blocks ytlo..ythi
-                const int ytlo = max((meta >> 8) & 0xff, 4 * half), ythi = min((meta >> 16) & 0xff, 4 * half + 3);
-                if (((meta >> plane) & 1) && ytlo <= ythi) {
+                const int ytlo = (meta >> 8) & 0xff, ythi = (meta >> 16) & 0xff;       // the touched 8-row blocks
+                if ((meta >> plane) & 1) {
                     double D1[NT][2][2];
 #pragma unroll
                     for (int nt = 0; nt < NT; ++nt) D1[nt][0][0] = D1[nt][0][1] = D1[nt][1][0] = D1[nt][1][1] = 0.0;
@@ -299,22 +300,21 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
                                 dmma(D1[nt][1][0], D1[nt][1][1], a, t2p[(size_t)kAddTZ * npp + t2off[nt][ks]]);
                             }
                     // A predicated-off DMMA still takes its 16 cycles of the pipe (measured), and the compiler
-                    // predicates a short "if": enter the unrolled blocks by a jump (eight cases make a jump table;
-                    // a warp only ever uses its four) and leave them by a branch instead.
+                    // predicates a short "if": enter the unrolled blocks by a jump and leave them by a branch instead.
 #define SHO_ADD_YBLOCK(YT)                                                                              \
     {                                                                                                   \
         double a_[KQ];                                                                                  \
         _Pragma("unroll") for (int kk = 0; kk < KQ; ++kk) a_[kk] = fxy[((YT) * KQ + kk) * 32];          \
         _Pragma("unroll") for (int kk = 0; kk < KQ; ++kk) {                                             \
-            dmma(D[(YT) & 3][0][0], D[(YT) & 3][0][1], a_[kk], D1[kk >> 1][0][kk & 1]);                 \
-            dmma(D[(YT) & 3][1][0], D[(YT) & 3][1][1], a_[kk], D1[kk >> 1][1][kk & 1]);                 \
+            dmma(D[YT][0][0], D[YT][0][1], a_[kk], D1[kk >> 1][0][kk & 1]);                 \
+            dmma(D[YT][1][0], D[YT][1][1], a_[kk], D1[kk >> 1][1][kk & 1]);                 \
         }                                                                                               \
     }
                     switch (ytlo) {
                         case 0: SHO_ADD_YBLOCK(0) if (ythi == 0) break;
                         case 1: SHO_ADD_YBLOCK(1) if (ythi == 1) break;
                         case 2: SHO_ADD_YBLOCK(2) if (ythi == 2) break;
-                        case 3: SHO_ADD_YBLOCK(3) break;
+                        case 3: SHO_ADD_YBLOCK(3) if (ythi == 3) break;
                         case 4: SHO_ADD_YBLOCK(4) if (ythi == 4) break;
                         case 5: SHO_ADD_YBLOCK(5) if (ythi == 5) break;
                         case 6: SHO_ADD_YBLOCK(6) if (ythi == 6) break;
@@ -333,7 +333,7 @@ __global__ void __launch_bounds__(kAddThreads, 1) sho_add_kernel(const __grid_co
             if (jz < Nz) {
                 const int jx = it.jx0 + 2 * t;
 #pragma unroll
-                for (int yt = 0; yt < 4; ++yt) {
+                for (int yt = 0; yt < NYT; ++yt) {
                     const int jy = row0 + 8 * yt + q;
                     if (jy < Ny && jx < Nx) {
                         if (CPLX) {
@@ -676,7 +676,7 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
     e = cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, pl->device);
     if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute(add)");
     const unsigned grid = (unsigned)std::min<long long>(nitems, std::max(nsm, 1));     // persistent: one CTA per SM
-    kern<<<grid, kAddThreads, smem, s>>>(p);
+    kern<<<grid, add_threads(CPLX), smem, s>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "launch sho_add_kernel");
     return SHO_OK;
