@@ -119,7 +119,11 @@ sho_status sho_project_stored(const sho_plan* plan, const sho_tables* tables, co
 /*
  * End-to-end variants with HOST buffers (pinned or pageable): copy in, run the same kernels, copy
  * out, and synchronise the stream before returning.  They use a device workspace owned by the plan
- * that is grown on demand (the only hot-path calls that may allocate).
+ * that is grown on demand (the only hot-path calls that may allocate).  The bands are independent
+ * (eq. (25)), so the calls work in chunks of bands (about 512 MB of psi each; environment
+ * variable SHO_HOST_CHUNK_BANDS overrides the chunk size) and overlap the H2D copy of the next chunk,
+ * the kernel of this one and the D2H copy of the previous one on two copy streams owned by the plan;
+ * all of it is ordered after the work already queued on cuda_stream.
  *   sho_project_host: psi HOST (read), coeff HOST (written)
  *   sho_add_host:     coeff HOST (read), psi HOST (in/out)
  */
