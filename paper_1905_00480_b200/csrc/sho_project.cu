@@ -165,6 +165,14 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
         }
     }
     const int KS = KX + (kdup != INT_MAX ? 1 : 0);
+    // row blocks that hold rows of a y image other than the home cell (the only ones whose phase is not 1)
+    int yrot_lo = 0, yrot_hi = -1;
+    if (yphase) {
+        const int mlo = floordiv(at.lo[1], Ny), mhi = floordiv(at.hi[1], Ny);
+        if (mlo != 0 && mhi != 0) { yrot_lo = 0; yrot_hi = NYB - 1; }
+        else if (mhi != 0) { yrot_lo = (Ny - at.lo[1]) >> 3; yrot_hi = NYB - 1; }
+        else if (mlo != 0) { yrot_lo = 0; yrot_hi = (-at.lo[1] - 1) >> 3; }
+    }
     const int KXG = (KS + G - 1) / G;
 
     // ---------------- a1: sample the 1D tables on the fly, in fragment layout ----------------
@@ -446,7 +454,7 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
                     for (int mt = 0; mt < MT; ++mt) { C1[mt][0][0] += C1[mt][1][0]; C1[mt][0][1] += C1[mt][1][1]; }
                 }
                 // ---- Bloch phase of each row (complex only): rotate the accumulators ----
-                if (yphase) {
+                if (yphase && yb >= yrot_lo && yb <= yrot_hi) {       // row blocks of the home image have phase 1
 #pragma unroll
                     for (int s = 0; s < 2; ++s) {
                         const double2 w = *reinterpret_cast<const double2*>(&wy[2 * (8 * yb + 2 * t + s)]);
