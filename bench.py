@@ -240,7 +240,7 @@ def run_ours(args, w):
     dom, t_dom = ("sho_add_kernel", t_add) if t_add >= t_prj else ("sho_project_kernel", t_prj)
     alu_peak = FP64_PEAK_TFLOPS                                      # arithmetic is fp64 for all four dtypes
     # dram__bytes_read + dram__bytes_write of one launch from the committed ncu --set full capture (cfg5 only)
-    traffic = {"sho_add_kernel": 8.285137e9 + 7.196659e9, "sho_project_kernel": 9.531631e9 + 0.235767e9}.get(dom) \
+    traffic = {"sho_add_kernel": 8.283107e9 + 7.196529e9, "sho_project_kernel": 9.560539e9 + 0.262074e9}.get(dom) \
         if (w.name == "cfg5" and w.dtype == "c128") else None
     roofline = {"bound": "alu", "kernel": dom, "achieved": F / t_dom / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
                 "frac": F / t_dom / 1e12 / alu_peak, "traffic": traffic,
