@@ -15,5 +15,7 @@ from .sho_oracle import (  # noqa: F401
     project_pairs,
     add,
     add_points,
+    add_points_bands,
+    dmul,
     num_threads,
 )

@@ -43,8 +43,10 @@
  *
  * Every function below is pinned by tests/test_oracle_pins.py (-m "not gpu") against things other
  * than itself: printed N_SHO values, scipy's Hermite polynomials, 1D orthonormality, separable ==
- * brute force, the closed-form Gaussian and plane-wave projections, the adjoint identity,
- * translation / zero-padding invariances.  Nothing here is "parity unpinned".
+ * brute force, the closed-form Gaussian and plane-wave projections (the Gaussian one also through
+ * the explicit-pair branch of oracle_project_pairs), the adjoint identity, translation / zero-padding
+ * invariances, a hand-written 2x2 product and numpy's matmul for oracle_dmul, Hermiticity of the
+ * three-step action.  Nothing here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -409,5 +411,117 @@ int oracle_add_points(const int32_t ng[3], double h, const int32_t periodic[3], 
         else { out[2 * s] = accre; out[2 * s + 1] = accim; }
     }
     free(lo); free(hi); free(empty);
+    return 0;
+}
+
+/*
+ * The same point-wise definition for SEVERAL bands of one grid point at once (sampled parity at full
+ * size over all bands: the 1D function values of a point do not depend on the band, so they are
+ * evaluated once per (point, atom image) and the sum over n runs per selected band):
+ *   out[s][k] = sum_a sum_{images} conj(w) sum_n c[a][band_sel[k]][n] phi_nx phi_ny phi_nz
+ * Same arithmetic, same order of the sums over atoms, images and n as oracle_add_points.
+ */
+int oracle_add_points_bands(const int32_t ng[3], double h, const int32_t periodic[3], const double* kfrac,
+                            int natoms, const double* pos, const double* sigma, int numax, double rcut_sigma,
+                            int is_complex, int nbands, const double* coeff,
+                            int64_t nsamples, const int32_t* pts /* [ns][3] = jx,jy,jz */,
+                            int nsel, const int32_t* band_sel /* [nsel] */,
+                            double* out /* [ns][nsel] (x2 if complex) */)
+{
+    int nsho = oracle_nsho(numax);
+    if (nsho < 0 || natoms < 0 || nbands <= 0 || h <= 0.0 || nsel <= 0) return 1;
+    for (int k = 0; k < nsel; ++k)
+        if (band_sel[k] < 0 || band_sel[k] >= nbands) return 1;
+    const size_t cw = is_complex ? 2 : 1;
+    int32_t* lo = (int32_t*)malloc(sizeof(int32_t) * 3 * (size_t)(natoms > 0 ? natoms : 1));
+    int32_t* hi = (int32_t*)malloc(sizeof(int32_t) * 3 * (size_t)(natoms > 0 ? natoms : 1));
+    int* empty = (int*)malloc(sizeof(int) * (size_t)(natoms > 0 ? natoms : 1));
+    for (int a = 0; a < natoms; ++a)
+        empty[a] = oracle_box(ng, h, periodic, pos + 3 * (size_t)a, sigma[a], rcut_sigma, lo + 3 * a, hi + 3 * a);
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t s = 0; s < nsamples; ++s) {
+        const int32_t* j = pts + 3 * s;
+        double* o = out + (size_t)s * nsel * cw;
+        for (size_t k = 0; k < (size_t)nsel * cw; ++k) o[k] = 0.0;
+        for (int a = 0; a < natoms; ++a) {
+            if (empty[a]) continue;
+            int m0[3], m1[3], skip = 0;
+            for (int d = 0; d < 3; ++d) {
+                if (periodic[d]) {
+                    m0[d] = (int)ceil(((double)lo[3 * a + d] - (double)j[d]) / (double)ng[d]);
+                    m1[d] = (int)floor(((double)hi[3 * a + d] - (double)j[d]) / (double)ng[d]);
+                } else {
+                    m0[d] = 0;
+                    m1[d] = (j[d] >= lo[3 * a + d] && j[d] <= hi[3 * a + d]) ? 0 : -1;
+                }
+                if (m1[d] < m0[d]) skip = 1;
+            }
+            if (skip) continue;
+            const double* R = pos + 3 * (size_t)a;
+            for (int mz = m0[2]; mz <= m1[2]; ++mz)
+                for (int my = m0[1]; my <= m1[1]; ++my)
+                    for (int mx = m0[0]; mx <= m1[0]; ++mx) {
+                        int m[3] = { mx, my, mz };
+                        double u[3];
+                        for (int d = 0; d < 3; ++d) u[d] = (double)(j[d] + m[d] * ng[d]) * h - R[d];
+                        double f[3][ORACLE_NUMAX_MAX + 1];   /* 1D values at this point, explicit formula */
+                        for (int d = 0; d < 3; ++d)
+                            for (int k = 0; k <= numax; ++k) f[d][k] = oracle_phi(k, u[d], sigma[a]);
+                        double ang = 2.0 * ORACLE_PI * (kfrac ? (kfrac[0] * mx + kfrac[1] * my + kfrac[2] * mz) : 0.0);
+                        double wr = cos(ang), wi = sin(ang);
+                        for (int k = 0; k < nsel; ++k) {
+                            const double* c = coeff + ((size_t)a * nbands + band_sel[k]) * nsho * cw;
+                            double vre = 0.0, vim = 0.0;
+                            int n = 0;
+                            for (int nz = 0; nz <= numax; ++nz)
+                                for (int ny = 0; ny <= numax - nz; ++ny)
+                                    for (int nx = 0; nx <= numax - nz - ny; ++nx) {
+                                        double p3 = f[2][nz] * f[1][ny] * f[0][nx];
+                                        if (!is_complex) vre += c[n] * p3;
+                                        else { vre += c[2 * n] * p3; vim += c[2 * n + 1] * p3; }
+                                        ++n;
+                                    }
+                            if (!is_complex) {
+                                o[k] += vre;
+                            } else {
+                                o[2 * k] += wr * vre + wi * vim;       /* conj(w) * v */
+                                o[2 * k + 1] += wr * vim - wi * vre;
+                            }
+                        }
+                    }
+        }
+    }
+    free(lo); free(hi); free(empty);
+    return 0;
+}
+
+/*
+ * Step (2) of the non-local action: "Multiplication: d^a_ik = sum_j D^a_ij c^a_jk", with the
+ * atomic matrix in the SHO representation, eq. (27)-(28) PAPER.md:252-262: "a real-valued matrix of
+ * dimension N_SHO" per atom.
+ *   D     [natoms][n][n]   real, row-major: D[a][i][j]
+ *   c, d  [natoms][nbands][n] (x2 doubles if is_complex), the layout of the coefficients (reading A9)
+ * Plain loops, one output at a time.
+ */
+int oracle_dmul(int natoms, int nbands, int n, int is_complex, const double* D, const double* c, double* d)
+{
+    if (natoms < 0 || nbands < 0 || n <= 0) return 1;
+    const size_t cw = is_complex ? 2 : 1;
+#pragma omp parallel for schedule(static)
+    for (int a = 0; a < natoms; ++a)
+        for (int b = 0; b < nbands; ++b) {
+            const double* cv = c + ((size_t)a * nbands + b) * (size_t)n * cw;
+            double* dv = d + ((size_t)a * nbands + b) * (size_t)n * cw;
+            for (int i = 0; i < n; ++i) {
+                double sre = 0.0, sim = 0.0;
+                for (int j = 0; j < n; ++j) {
+                    double Dij = D[((size_t)a * n + i) * (size_t)n + j];
+                    if (!is_complex) sre += Dij * cv[j];
+                    else { sre += Dij * cv[2 * j]; sim += Dij * cv[2 * j + 1]; }
+                }
+                if (!is_complex) dv[i] = sre;
+                else { dv[2 * i] = sre; dv[2 * i + 1] = sim; }
+            }
+        }
     return 0;
 }

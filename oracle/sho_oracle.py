@@ -54,6 +54,8 @@ def _load():
         lib.oracle_project_pairs.argtypes = common + [_f64p, C.POINTER(_f64p), C.c_int64, _i32p, _i32p, _f64p]
         lib.oracle_add.argtypes = common + [_f64p, _f64p]
         lib.oracle_add_points.argtypes = common + [_f64p, C.c_int64, _i32p, _i32p, _f64p]
+        lib.oracle_dmul.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, _f64p, _f64p, _f64p]
+        lib.oracle_add_points_bands.argtypes = common + [_f64p, C.c_int64, _i32p, C.c_int, _i32p, _f64p]
         _lib = lib
     return _lib
 
@@ -185,4 +187,34 @@ def add_points(ng, h, periodic, kfrac, pos, sigma, numax, coeff, pts, bands, rcu
                                    _p(out.view(np.float64), _f64p))
     assert rc == 0, "oracle_add_points failed"
     del keep
+    return out
+
+
+def add_points_bands(ng, h, periodic, kfrac, pos, sigma, numax, coeff, pts, band_sel, rcut_sigma=6.0):
+    """(A c)(r_j) -- the increment only -- at sample points pts[ns][3] = (jx,jy,jz) for every band in
+    ``band_sel``: out[ns][len(band_sel)]."""
+    is_complex = np.iscomplexobj(coeff)
+    c_, c_r = _as_real_view(coeff, is_complex)
+    nb = c_.shape[1]
+    args, keep = _common(ng, h, periodic, kfrac, pos, sigma, numax, rcut_sigma, is_complex, nb)
+    pts_, b_ = _i32(pts).reshape(-1, 3), _i32(band_sel).reshape(-1)
+    out = np.zeros((len(pts_), len(b_)), dtype=np.complex128 if is_complex else np.float64)
+    rc = _load().oracle_add_points_bands(*args, _p(c_r, _f64p), len(pts_), _p(pts_, _i32p), len(b_), _p(b_, _i32p),
+                                         _p(out.view(np.float64), _f64p))
+    assert rc == 0, "oracle_add_points_bands failed"
+    del keep
+    return out
+
+
+def dmul(D, coeff):
+    """Step (2): d[a][b][i] = sum_j D[a][i][j] c[a][b][j]; D real [natoms][n][n]."""
+    is_complex = np.iscomplexobj(coeff)
+    c_, c_r = _as_real_view(coeff, is_complex)
+    D_ = _f64(D)
+    na, nb, n = c_.shape
+    assert D_.shape == (na, n, n)
+    out = np.zeros_like(c_)
+    rc = _load().oracle_dmul(na, nb, n, int(is_complex), _p(D_, _f64p), _p(c_r, _f64p),
+                             _p(out.view(np.float64) if is_complex else out, _f64p))
+    assert rc == 0, "oracle_dmul failed"
     return out

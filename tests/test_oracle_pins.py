@@ -455,3 +455,143 @@ def test_degenerate_cases():
     c = oracle.project((16, 16, 16), 0.25, (1, 1, 1), None, np.array([[2.0, 2.1, 1.9]]), np.array([0.4]), 0,
                        np.ones((1, 16, 16, 16)), rcut_sigma=8.0)
     assert c[0, 0, 0] == pytest.approx((math.sqrt(2) * math.pi ** 0.25 * math.sqrt(0.4)) ** 3, rel=1e-12)
+
+
+# ----------------------------------------------------------------------------------------------
+# the explicit-pair branch of oracle_project_pairs (pair_atom / pair_band lists, bands in separate
+# buffers through psi_band_ptrs): every full-size GPU parity check rests on it
+
+
+def test_project_pairs_explicit_branch_gaussian_closed_form():
+    """P3 through the explicit-pair branch: two atoms, three bands held in SEPARATE buffers, a shuffled pair
+    list with a repeated pair; band 1 is an off-centre Gaussian around atom 1 whose coefficients have the
+    closed form of test_P3_gaussian_projection_general, band 2 one around atom 0 (transposed atom / band
+    indices, a wrong output row or a wrong band pointer all fail)."""
+    ng, h, numax = (72, 80, 64), 0.2, 4
+    sigma = np.array([0.8, 0.7])
+    R = np.array([[7.13, 8.02, 6.31], [7.49, 7.77, 6.58]])
+    s = [None, 0.6, 0.75]
+    d = [None, np.array([0.21, -0.32, 0.17]), np.array([-0.25, 0.14, 0.33])]
+    centre = [None, R[1] + d[1], R[0] + d[2]]
+    rng = np.random.default_rng(21)
+    bands = {0: rng.standard_normal((ng[2], ng[1], ng[0]))}
+    for b in (1, 2):
+        ax = [np.arange(ng[k]) * h - centre[b][k] for k in range(3)]
+        bands[b] = np.exp(-0.5 * (ax[2][:, None, None] ** 2 + ax[1][None, :, None] ** 2 + ax[0][None, None, :] ** 2) / s[b] ** 2)
+    pa = np.array([1, 0, 1, 0, 1])
+    pb = np.array([1, 2, 0, 0, 1])
+    c = oracle.project_pairs(ng, h, (0, 0, 0), None, R, sigma, numax, bands, pa, pb, 3, False, rcut_sigma=8.5)
+    assert c.shape == (5, oracle.nsho(numax))
+    for row, (a, b) in ((0, (1, 1)), (1, (0, 2)), (4, (1, 1))):
+        one = [[gaussian_overlap_1d(n, sigma[a], s[b], d[b][k]) for n in range(numax + 1)] for k in range(3)]
+        for nz in range(numax + 1):
+            for ny in range(numax + 1 - nz):
+                for nx in range(numax + 1 - nz - ny):
+                    ref = one[0][nx] * one[1][ny] * one[2][nz]
+                    assert c[row, oracle.index(nx, ny, nz, numax)] == pytest.approx(ref, rel=1e-10, abs=2e-13)
+    assert np.array_equal(c[0], c[4])
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+def test_project_pairs_explicit_branch_equals_rows_of_full_projection(cplx):
+    """A shuffled subset of (atom, band) pairs, bands passed as separate buffers, equals the matching rows
+    of the full projection (wrap, Bloch phase) and of the separable numpy contraction with scipy tables."""
+    rng = np.random.default_rng(22)
+    ng, h, per = (18, 22, 20), 0.3, (1, 1, 1)
+    kfrac = (0.1, 0.2, 0.3) if cplx else None
+    pos = rng.uniform(0, 1, size=(5, 3)) * np.array(ng) * h
+    sigma = rng.uniform(0.3, 0.4, size=5)
+    numax, nb = 3, 4
+    shape = (nb, ng[2], ng[1], ng[0])
+    psi = rng.standard_normal(shape) + (1j * rng.standard_normal(shape) if cplx else 0)
+    full = oracle.project(ng, h, per, kfrac, pos, sigma, numax, psi, rcut_sigma=5.0)
+    sep = separable_project(ng, h, per, kfrac, pos, sigma, numax, psi, 5.0)
+    pairs = [(a, b) for a in range(5) for b in range(nb)]
+    sel = rng.permutation(len(pairs))[:11]
+    pa = np.array([pairs[i][0] for i in sel])
+    pb = np.array([pairs[i][1] for i in sel])
+    bands = {int(b): psi[int(b)].copy() for b in np.unique(pb)}      # separate buffers, only the bands in use
+    got = oracle.project_pairs(ng, h, per, kfrac, pos, sigma, numax, bands, pa, pb, nb, cplx, rcut_sigma=5.0)
+    assert np.array_equal(got, full[pa, pb])
+    assert np.max(np.abs(got - sep[pa, pb])) < 1e-13 * np.max(np.abs(sep))
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+def test_add_points_bands_matches_full_add(cplx):
+    """The all-bands point-wise evaluation equals the box-loop add (multi-image boxes, Bloch phase, an
+    isolated axis) for a subset of bands given in a shuffled order."""
+    rng = np.random.default_rng(23)
+    ng, h, per = (14, 16, 12), 0.3, (1, 1, 0)
+    kfrac = (0.1, 0.2, 0.0) if cplx else None
+    pos = rng.uniform(0, 1, size=(3, 3)) * np.array(ng) * h
+    sigma = np.array([0.3, 0.38, 0.45])
+    numax, nb = 3, 5
+    cshape = (3, nb, oracle.nsho(numax))
+    c = rng.standard_normal(cshape) + (1j * rng.standard_normal(cshape) if cplx else 0)
+    full = oracle.add(ng, h, per, kfrac, pos, sigma, numax, c, np.zeros((nb, ng[2], ng[1], ng[0]), dtype=c.dtype))
+    pts = np.stack([rng.integers(0, ng[0], 150), rng.integers(0, ng[1], 150), rng.integers(0, ng[2], 150)], axis=1)
+    sel = np.array([4, 0, 2])
+    got = oracle.add_points_bands(ng, h, per, kfrac, pos, sigma, numax, c, pts, sel)
+    ref = full[sel][:, pts[:, 2], pts[:, 1], pts[:, 0]].T
+    assert got.shape == (150, 3)
+    assert np.max(np.abs(got - ref)) < 1e-13 * max(1.0, np.max(np.abs(ref)))
+
+
+# ----------------------------------------------------------------------------------------------
+# step (2): d = D c  (PAPER.md:189, eq. (27)-(28) PAPER.md:252-262)
+
+
+def test_dmul_hand_written_2x2_and_identity():
+    # d_i = sum_j D_ij c_j with D = [[2, -1], [3, 0.5]] (NOT symmetric: a transposed D fails), two bands
+    D = np.array([[[2.0, -1.0], [3.0, 0.5]]])
+    c = np.array([[[1.0, 4.0], [-2.0, 0.25]]])
+    d = oracle.dmul(D, c)
+    assert np.array_equal(d, np.array([[[2.0 * 1 - 1.0 * 4, 3.0 * 1 + 0.5 * 4], [2.0 * -2 - 0.25, 3.0 * -2 + 0.125]]]))
+    cz = c + 1j * np.array([[[0.5, -1.0], [2.0, 8.0]]])
+    dz = oracle.dmul(D, cz)
+    assert np.array_equal(dz.real, d)
+    assert np.array_equal(dz.imag, np.array([[[2.0 * 0.5 + 1.0, 3.0 * 0.5 - 0.5], [2.0 * 2 - 8.0, 3.0 * 2 + 4.0]]]))
+    rng = np.random.default_rng(24)
+    c = rng.standard_normal((3, 2, 10))
+    assert np.array_equal(oracle.dmul(np.tile(np.eye(10), (3, 1, 1)), c), c)
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+def test_dmul_matches_library_matmul_per_atom(cplx):
+    rng = np.random.default_rng(25)
+    na, nb, n = 4, 3, oracle.nsho(3)
+    D = rng.standard_normal((na, n, n))
+    c = rng.standard_normal((na, nb, n)) + (1j * rng.standard_normal((na, nb, n)) if cplx else 0)
+    ref = np.einsum("aij,abj->abi", D, c)
+    assert np.max(np.abs(oracle.dmul(D, c) - ref)) < 1e-13 * np.max(np.abs(ref))
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+def test_nonlocal_action_is_hermitian_for_symmetric_D(cplx):
+    """V = A D P (steps (1)-(3)) with real symmetric D per atom is Hermitian:
+    <phi, V psi> = conj(<psi, V phi>) (grid inner product; add = P^H / h^3, reading A7).  With D = 1 the
+    action reduces to add(project(psi))."""
+    rng = np.random.default_rng(26)
+    ng, h, per = (18, 16, 20), 0.3, (1, 1, 1)
+    kfrac = (0.15, -0.2, 0.35) if cplx else None
+    pos = rng.uniform(0, 1, size=(3, 3)) * np.array(ng) * h
+    sigma = rng.uniform(0.3, 0.4, size=3)
+    numax = 3
+    n = oracle.nsho(numax)
+    D = rng.standard_normal((3, n, n))
+    D = D + np.transpose(D, (0, 2, 1))
+    shape = (1, ng[2], ng[1], ng[0])
+    psi = rng.standard_normal(shape) + (1j * rng.standard_normal(shape) if cplx else 0)
+    phi = rng.standard_normal(shape) + (1j * rng.standard_normal(shape) if cplx else 0)
+
+    def V(f, Dm):
+        c = oracle.project(ng, h, per, kfrac, pos, sigma, numax, f, rcut_sigma=5.0)
+        return oracle.add(ng, h, per, kfrac, pos, sigma, numax, oracle.dmul(Dm, c), np.zeros_like(f), rcut_sigma=5.0)
+
+    lhs = np.sum(np.conj(phi) * V(psi, D))
+    rhs = np.conj(np.sum(np.conj(psi) * V(phi, D)))
+    assert abs(lhs - rhs) < 1e-12 * abs(lhs)
+    one = np.tile(np.eye(n), (3, 1, 1))
+    c = oracle.project(ng, h, per, kfrac, pos, sigma, numax, psi, rcut_sigma=5.0)
+    ref = oracle.add(ng, h, per, kfrac, pos, sigma, numax, c, np.zeros_like(psi), rcut_sigma=5.0)
+    assert np.array_equal(V(psi, one), ref)
