@@ -33,7 +33,10 @@
  * (sho_project, sho_add, sho_project_stored) allocate nothing, are asynchronous on the given CUDA
  * stream and never synchronise the host.  psi must be finite on the whole grid (values just outside
  * a box are multiplied by exact zeros).  There is no CPU fallback: without a CUDA device every call
- * that needs one returns SHO_ERR_CUDA.
+ * that needs one returns SHO_ERR_CUDA.  A plan belongs to the CUDA device that was current when it was
+ * created: every hot call checks that this device is current and returns SHO_ERR_INVALID_ARG otherwise.
+ * The only device-side abort is a watchdog: a kernel-internal barrier wait longer than 30 s of wall
+ * time (a lost arrival, i.e. a library bug) traps, which the host sees as SHO_ERR_CUDA.
  */
 #ifndef SHO_H_
 #define SHO_H_
@@ -102,7 +105,9 @@ sho_status sho_plan_info(const sho_plan* plan, int64_t info[8]);
 sho_status sho_project(const sho_plan* plan, const void* psi, int32_t nbands, void* coeff, void* cuda_stream);
 
 /* Expansion / add-back, on-the-fly SHO: psi += A coeff.  coeff DEVICE (read), psi DEVICE (in/out).
- * Deterministic: every psi value is accumulated by exactly one thread, atoms in ascending order. */
+ * Deterministic: every psi value is accumulated by exactly one thread, the (atom, image) terms in the
+ * fixed order of the plan's tile lists inside FP64 MMA accumulators, then added to psi once: two runs
+ * give bit-identical results (the order is not "atoms ascending, one by one"). */
 sho_status sho_add(const sho_plan* plan, const void* coeff, int32_t nbands, void* psi, void* cuda_stream);
 
 /*
@@ -131,7 +136,8 @@ sho_status sho_project_host(sho_plan* plan, const void* psi_host, int32_t nbands
 sho_status sho_add_host(sho_plan* plan, const void* coeff_host, int32_t nbands, void* psi_host, void* cuda_stream);
 
 /* FP64 FMA-pipe micro-benchmark used by bench.py for the roofline denominator: runs `iters` rounds of
- * dependent DMMA chains on every SM and returns the achieved FLOP/s in *flops_per_s (synchronises). */
+ * eight independent DFMA chains per thread on every SM and returns the achieved FLOP/s in *flops_per_s
+ * (synchronises).  DMMA.8x8x4 shares that pipe at the same rate. */
 sho_status sho_measure_fp64_peak(int32_t iters, double* flops_per_s);
 
 #ifdef __cplusplus

@@ -9,15 +9,17 @@
 // tile and finally does ONE read-modify-write of the tile.  No atomics, bit-reproducible, psi traffic =
 // read + write of every touched tile exactly once.
 //
-// The CTA is warp-specialised; the three roles are coupled only by mbarrier rings, never by a CTA barrier:
-//   T warps (4)   per pair: the three 1D Hermite-Gauss tables, sampled on the fly (eq. (31))
-//                 into shared memory in MMA fragment order (shared by both channels), and the pair's
-//                 coefficients c[a][b][:] (prefetched one pair ahead, records of the pair list three pairs
-//                 ahead by cp.async), times the conjugate Bloch phase of the image, scattered into the A
-//                 fragments of the z stage
-//   Z warps (4)   z stage   T2[z][(ny,nx)] = sum_nz c[n(nx,ny,nz)] phi_nz(z)    M = (ny,nx) pairs sorted by
-//                 ny+nx (row tile mt needs only nz <= numax - s_min(mt)), K = nz, N = the 8 planes
-//   XY warps (16) warp (plane, channel) owns 64 rows x 8 columns of one plane of one channel:
+// The CTA is persistent and warp-specialised; the two roles are coupled only by an mbarrier ring, never by a
+// CTA barrier:
+//   producer warps (8)  warp w builds pairs w, w + 8, ... entirely on its own: the pair's record and its
+//                 coefficients c[a][b][:] (cp.async, each lane copying exactly the A-fragment elements it will
+//                 feed to the z-stage MMAs), the three 1D Hermite-Gauss tables sampled on the fly (eq. (31),
+//                 PAPER.md:283-286) into shared memory in MMA fragment order (shared by both channels), then the
+//                 z stage   T2[z][(ny,nx)] = sum_nz c[n(nx,ny,nz)] phi_nz(z)    M = (ny,nx) pairs sorted by
+//                 ny+nx (row tile mt needs only nz <= numax - s_min(mt)), K = nz, N = the 8 planes,
+//                 with the conjugate Bloch phase of the image applied to the A elements
+//   XY warps (8 complex / 16 real)  a warp owns 64 rows x 8 columns of one plane (both channels for complex
+//                 data, one channel for real data):
 //                 x stage   T1[x][ny]  = sum_nx phi_nx(x) T2[z][(ny,nx)]        M = x, K = nx, N = ny
 //                 y stage   psi[y][x] += sum_ny phi_ny(y) T1[x][ny]             M = y, K = ny, N = x
 //                 The accumulator fragment of the x stage is exactly the B fragment of the y stage when

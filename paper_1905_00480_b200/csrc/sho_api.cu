@@ -3,6 +3,7 @@
 // add), the HOST-buffer end-to-end variants and the FP64 micro-benchmark.  All arithmetic of the hot
 // path lives in the kernels (sho_project.cu, sho_add.cu, sho_stored.cu).
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -131,6 +132,10 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
     p->s_in = nullptr; p->s_out = nullptr;
     p->rcut_sigma = rcut_sigma;
     p->dtype = dtype;
+    {
+        static std::atomic<uint64_t> next_serial{1};
+        p->serial = next_serial.fetch_add(1);
+    }
     std::memset(&p->g, 0, sizeof(p->g));
     GridDev& g = p->g;
     for (int d = 0; d < 3; ++d) {
@@ -423,6 +428,13 @@ static sho_status check_hot(const char* fn, const sho_plan* plan, const void* a,
 {
     if (!plan || !a || !b) { set_error("%s: null argument", fn); return SHO_ERR_INVALID_ARG; }
     if (nbands <= 0) { set_error("%s: nbands must be > 0", fn); return SHO_ERR_INVALID_ARG; }
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, fn);
+    if (dev != plan->device) {
+        set_error("%s: the plan belongs to CUDA device %d but device %d is current", fn, plan->device, dev);
+        return SHO_ERR_INVALID_ARG;
+    }
     return SHO_OK;
 }
 
@@ -464,10 +476,10 @@ sho_status sho_tables_destroy(sho_tables* t)
 sho_status sho_project_stored(const sho_plan* plan, const sho_tables* tables, const void* psi, int32_t nbands,
                               void* coeff, void* cuda_stream)
 {
-    if (plan && plan->g.natoms == 0 && psi && nbands > 0 && tables && tables->plan == plan) return SHO_OK;
+    if (plan && plan->g.natoms == 0 && psi && nbands > 0 && tables && tables->plan == plan && tables->plan_serial == plan->serial) return SHO_OK;
     sho_status st = check_hot("sho_project_stored", plan, psi, coeff, nbands);
     if (st != SHO_OK) return st;
-    if (!tables || tables->plan != plan) { set_error("sho_project_stored: tables do not belong to this plan"); return SHO_ERR_INVALID_ARG; }
+    if (!tables || tables->plan != plan || tables->plan_serial != plan->serial) { set_error("sho_project_stored: tables do not belong to this plan"); return SHO_ERR_INVALID_ARG; }
     return launch_project_stored(plan, tables, psi, nbands, coeff, static_cast<cudaStream_t>(cuda_stream));
 }
 

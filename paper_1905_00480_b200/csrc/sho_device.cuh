@@ -26,16 +26,39 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
 }
-// wait until the phase with this parity has completed; a wait that never ends traps instead of hanging the GPU
+// Wait until the phase with this parity has completed.  try_wait suspends the thread for a hardware-chosen
+// time slice, so the loop is not a hot spin.  A wait that lasts longer than kMbarTimeoutNs of wall time (a
+// lost arrival: a bug, not a slow run -- compute-sanitizer or a debugger stretch a wait by far less) traps
+// instead of hanging the GPU; the host then sees SHO_ERR_CUDA from the next runtime call on that context.
+constexpr unsigned long long kMbarTimeoutNs = 30ull * 1000000000ull;
+__device__ __forceinline__ unsigned long long global_timer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t a, int parity)
+{
+    uint32_t done;
+    asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.b32 %0, 1, 0, p;\n}\n"
+                 : "=r"(done) : "r"(a), "r"((uint32_t)parity) : "memory");
+    return done != 0;
+}
+static __device__ __noinline__ void mbar_wait_slow(uint32_t a, int parity)
+{
+    const unsigned long long t0 = global_timer_ns();
+    for (;;) {
+        for (int spin = 0; spin < 4096; ++spin)
+            if (mbar_try_wait(a, parity)) return;
+        if (global_timer_ns() - t0 > kMbarTimeoutNs) __trap();
+    }
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, int parity)
 {
     const uint32_t a = (uint32_t)__cvta_generic_to_shared(bar);
-    uint32_t done = 0;
-    for (long long spin = 0; !done; ++spin) {
-        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.b32 %0, 1, 0, p;\n}\n"
-                     : "=r"(done) : "r"(a), "r"((uint32_t)parity) : "memory");
-        if (spin > (1LL << 26)) __trap();
-    }
+    if (mbar_try_wait(a, parity)) return;
+    if (mbar_try_wait(a, parity)) return;
+    mbar_wait_slow(a, parity);
 }
 
 __device__ __forceinline__ int floordiv(int i, int n)

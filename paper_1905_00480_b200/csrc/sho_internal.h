@@ -72,6 +72,7 @@ struct sho_plan {
     double rcut_sigma;
     sho_dtype dtype;
     int device;
+    uint64_t serial;                       // unique per plan (a new plan at a recycled address is a different plan)
     std::vector<sho::AtomDev> atoms;       // host copy, original order
     std::vector<int32_t> order;            // spatially sorted atom indices (non-empty boxes first)
     int32_t n_nonempty;
@@ -104,6 +105,7 @@ struct sho_plan {
 
 struct sho_tables {
     const sho_plan* plan;
+    uint64_t plan_serial;
     void* d_data;                          // fragment-ordered tables, see sho_stored.cu
     int64_t* d_atom_off;                   // [natoms+1] offsets in elements
     int32_t* d_seg_atom;                   // K segments (atom, first box plane) = the CTAs of the stored kernel

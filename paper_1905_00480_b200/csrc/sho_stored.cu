@@ -238,7 +238,7 @@ sho_status tables_build(const sho_plan* pl, sho_tables** out, size_t* bytes_need
     }
     sho_tables* t = new (std::nothrow) sho_tables();
     if (!t) { set_error("sho_tables_build: host allocation failed"); return SHO_ERR_OOM; }
-    t->plan = pl; t->d_data = nullptr; t->d_atom_off = nullptr; t->d_seg_atom = nullptr; t->d_seg_qz0 = nullptr;
+    t->plan = pl; t->plan_serial = pl->serial; t->d_data = nullptr; t->d_atom_off = nullptr; t->d_seg_atom = nullptr; t->d_seg_qz0 = nullptr;
     t->atom_off = off; t->bytes = *bytes_needed; t->nseg = (int32_t)seg_atom.size();
     int32_t *d_pa = nullptr, *d_pq = nullptr;
     auto fail = [&](sho_status st) { cudaFree(d_pa); cudaFree(d_pq); cudaFree(t->d_seg_atom); cudaFree(t->d_seg_qz0);

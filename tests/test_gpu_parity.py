@@ -235,15 +235,42 @@ def test_bloch_image_boundary_inside_a_load_step(sho, nx):
     run_case(sho, _custom(ng, (1, 1, 1), pos, [0.3, 0.34, 0.32], 6, 3, dtype="c64", kfrac=(0.17, -0.2, 0.3), rc=5.0))
 
 
-@pytest.mark.parametrize("k", [3, 4, 5])
-def test_full_size_config_sampled(sho, k):
+def _sample_atoms(w, boxes):
+    """Atoms for sampled full-size parity: boxes that wrap on all three axes, the sigma extremes, interior
+    boxes (no wrap at all), the first and the last atom -- at least 8 distinct atoms."""
+    ng = np.array(w.ng)
+    wrap_all = [a for a in range(w.natoms) if all(boxes[a, d, 0] < 0 or boxes[a, d, 1] >= ng[d] for d in range(3))]
+    wrap_none = [a for a in range(w.natoms) if all(boxes[a, d, 0] >= 0 and boxes[a, d, 1] < ng[d] for d in range(3))]
+    wrap_some = [a for a in range(w.natoms) if a not in wrap_all and a not in wrap_none]
+    pick = wrap_all[:3] + wrap_none[:2] + wrap_some[:2] + [int(np.argmin(w.sigma)), int(np.argmax(w.sigma)), 0, w.natoms - 1]
+    atoms = []
+    for a in pick + list(range(w.natoms)):
+        if a not in atoms:
+            atoms.append(a)
+        if len(atoms) >= 8 and all(x in atoms for x in pick):
+            break
+    return atoms
+
+
+def _sample_bands(nb, n=8):
+    """First, last and interior bands (the add kernel's work item index runs over bands)."""
+    return sorted(set([0, 1, nb // 3, nb // 2 - 1, nb // 2, (2 * nb) // 3 + 1, nb - 2, nb - 1][:n]) & set(range(nb)))
+
+
+@pytest.mark.parametrize("k,dtype", [(3, None), (4, None), (4, "r32"), (5, None)])
+def test_full_size_config_sampled(sho, k, dtype):
     """BASELINE.json config k at its full size, in the launch configuration bench.py times (all bands, device
-    inputs from a seeded torch generator): project checked on sampled (atom, band) pairs -- atoms whose box
-    wraps on every axis, the smallest and the largest sigma -- and add on 2 z-planes' worth of random points
-    of the first and the last band, each computed one by one by the oracle (reading A13 norms; the add scale
-    is the largest reference increment among the samples)."""
+    inputs from a seeded torch generator), sampled as SURVEY 8(d) asks:
+      project: >= 64 (atom, band) pairs -- atoms whose box wraps on every axis, on none, the smallest and the
+               largest sigma -- over 8 bands including interior ones, each computed by the oracle's direct sum;
+      stored-projector project (cfg 3, the config it is timed on): the same pairs;
+      add:     into a NON-ZERO psi: four full z-planes (0, Nz-1, the first plane of the second tile layer, a
+               middle plane) for 8 bands, plus 4096 random points for ALL bands, every value computed
+               point-wise by the oracle.  Norms of reading A13 over the samples."""
     import torch
-    w = workloads.make(k)
+    w = workloads.make(k, dtype=dtype)
+    if dtype in ("r32", "r64"):
+        w.kfrac = None
     tol = TOL[w.dtype]
     wide = np.complex128 if w.is_complex else np.float64
     tdt = {"r64": torch.float64, "c128": torch.complex128, "r32": torch.float32, "c64": torch.complex64}[w.dtype]
@@ -258,35 +285,57 @@ def test_full_size_config_sampled(sho, k):
         c_gpu = plan.project(psi)
         torch.cuda.synchronize()
         # ---- project: sampled pairs ----
-        ng = np.array(w.ng)
-        wraps = [a for a in range(w.natoms) if all(boxes[a, d, 0] < 0 or boxes[a, d, 1] >= ng[d] for d in range(3))]
-        atoms = sorted(set(wraps[:3] + [int(np.argmin(w.sigma)), int(np.argmax(w.sigma)), 0, w.natoms - 1]))
-        pairs = [(a, b) for a in atoms for b in (0, w.nbands - 1)]
-        bands = {b: psi[b].cpu().numpy().astype(wide) for b in (0, w.nbands - 1)}
+        atoms = _sample_atoms(w, boxes)
+        bsel = _sample_bands(w.nbands)
+        pairs = [(a, b) for a in atoms for b in bsel]
+        assert len(pairs) >= 64 and len(bsel) >= 8
+        bands = {b: psi[b].cpu().numpy().astype(wide) for b in bsel}
         pa, pb = np.array([q[0] for q in pairs]), np.array([q[1] for q in pairs])
         ref = oracle.project_pairs(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax, bands, pa, pb, w.nbands,
                                    w.is_complex, w.rcut_sigma)
         norm = np.array([np.sqrt(w.h ** 3 * np.sum(np.abs(bands[int(b)]) ** 2)) for b in pb])
-        got = c_gpu[torch.as_tensor(pa, device="cuda"), torch.as_tensor(pb, device="cuda")].cpu().numpy().astype(wide)
+        ia, ib = torch.as_tensor(pa, device="cuda"), torch.as_tensor(pb, device="cuda")
+        got = c_gpu[ia, ib].cpu().numpy().astype(wide)
         err = (np.abs(got - ref) / norm[:, None]).max()
         assert err <= tol, "project parity at full size: %.3e > %.1e" % (err, tol)
-        del psi
-        # ---- add: sampled points ----
+        # ---- stored-projector baseline at the size it is timed on (cfg 3: 53 GB of tables) ----
+        if k == 3:
+            tb = plan.tables()
+            c_sto = plan.project_stored(tb, psi)
+            torch.cuda.synchronize()
+            got = c_sto[ia, ib].cpu().numpy().astype(wide)
+            tb.close()
+            err = (np.abs(got - ref) / norm[:, None]).max()
+            assert err <= tol, "stored-projector parity at full size: %.3e > %.1e" % (err, tol)
+            del c_sto
+        # ---- add into the non-zero psi: full planes of 8 bands + random points of all bands ----
         coeff = torch.randn((w.natoms, w.nbands, plan.nsho), dtype=tdt, device="cuda", generator=gen)
-        out = torch.zeros(shape, dtype=tdt, device="cuda")
-        plan.add(coeff, out)
+        psi0 = psi.clone()
+        plan.add(coeff, psi)
         torch.cuda.synchronize()
+        coeff_h = coeff.cpu().numpy().astype(wide)
+        Nx, Ny, Nz = w.ng
+        worst = 0.0
+        for jz in (0, Nz - 1, 8, Nz // 2 + 3):
+            yy, xx = np.meshgrid(np.arange(Ny), np.arange(Nx), indexing="ij")
+            pts = np.stack([xx.ravel(), yy.ravel(), np.full(xx.size, jz)], axis=1)
+            inc = oracle.add_points_bands(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax, coeff_h, pts, bsel,
+                                          w.rcut_sigma)                                   # [Ny*Nx][8]
+            tb_ = torch.as_tensor(bsel, device="cuda")
+            refp = psi0[tb_, jz].cpu().numpy().astype(wide).reshape(len(bsel), -1).T + inc
+            gotp = psi[tb_, jz].cpu().numpy().astype(wide).reshape(len(bsel), -1).T
+            e = (np.abs(gotp - refp).max(axis=0) / np.abs(refp).max(axis=0)).max()
+            worst = max(worst, float(e))
+            assert e <= tol, "add parity at full size, plane z = %d: %.3e > %.1e" % (jz, e, tol)
         rng = np.random.default_rng(w.seed)
-        ns = 2 * w.ng[0] * w.ng[1] // 8
-        pts = np.stack([rng.integers(0, w.ng[d], ns) for d in range(3)], axis=1)
-        pts[: ns // 4, 2] = 0                       # a quarter of them on the first plane (wrapped boxes)
-        bsel = np.where(rng.integers(0, 2, ns) == 0, 0, w.nbands - 1)
-        refp = oracle.add_points(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax,
-                                 coeff.cpu().numpy().astype(wide), pts, bsel, w.rcut_sigma)
-        gotp = out[torch.as_tensor(bsel, device="cuda"), torch.as_tensor(pts[:, 2], device="cuda"),
-                   torch.as_tensor(pts[:, 1], device="cuda"), torch.as_tensor(pts[:, 0], device="cuda")].cpu().numpy().astype(wide)
-        erra = np.abs(gotp - refp).max() / np.abs(refp).max()
-        assert erra <= tol, "add parity at full size: %.3e > %.1e" % (erra, tol)
+        pts = np.stack([rng.integers(0, w.ng[d], 4096) for d in range(3)], axis=1)
+        allb = np.arange(w.nbands)
+        inc = oracle.add_points_bands(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax, coeff_h, pts, allb, w.rcut_sigma)
+        iz, iy, ix = (torch.as_tensor(pts[:, d], device="cuda") for d in (2, 1, 0))
+        refp = psi0[:, iz, iy, ix].cpu().numpy().astype(wide).T + inc
+        gotp = psi[:, iz, iy, ix].cpu().numpy().astype(wide).T
+        e = (np.abs(gotp - refp).max(axis=0) / np.abs(refp).max(axis=0)).max()
+        assert e <= tol, "add parity at full size, random points of all bands: %.3e > %.1e" % (e, tol)
     finally:
         plan.close()
 
