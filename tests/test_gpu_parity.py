@@ -391,6 +391,89 @@ def test_add_is_bit_reproducible(sho):
     plan.close()
 
 
+@pytest.mark.parametrize("name", ["cfg2-small", "cfg5-small", "ragged"])
+def test_no_write_outside_the_callers_buffers(sho, name):
+    """compute-sanitizer is closed on this pool (profiles/r2_sanitizer.md), so out-of-bounds WRITES are caught here:
+    psi and coeff live inside larger allocations whose guard zones (64 KB on each side, a NaN bit pattern) must come
+    back untouched from project, add, the stored-projector project and the fused action; reads outside the buffers
+    would hit NaNs and fail the finiteness / parity checks of the other tests."""
+    import torch
+    if name == "ragged":
+        rng = np.random.default_rng(3)
+        ng = (33, 37, 29)
+        w = _custom(ng, (1, 0, 1), rng.uniform(0, 1, (5, 3)) * np.array(ng) * 0.25, rng.uniform(0.35, 0.6, 5), 9, 3,
+                    dtype="c128", kfrac=(0.1, 0.0, 0.3))
+    else:
+        w = workloads.make(int(name[3]), size="small")
+    plan = sho.plan_for(w)
+    G = 8192                                     # guard elements (64 KB of fp64)
+    tdt = torch.complex128 if w.is_complex else torch.float64
+
+    def guarded(shape):
+        n = int(np.prod(shape))
+        buf = torch.full((n + 2 * G,), float("nan"), dtype=tdt, device="cuda")
+        return buf, buf[G:G + n].view(shape)
+
+    def intact(buf, n):
+        g = torch.view_as_real(buf) if w.is_complex else buf
+        k = 2 if w.is_complex else 1
+        return bool(torch.isnan(g[:G * k]).all()) and bool(torch.isnan(g[(G + n) * k:]).all())
+
+    try:
+        psi_h = w.psi()
+        if w.psi_dist == "zero":
+            psi_h = workloads.Workload(**{**w.__dict__, "psi_dist": "normal"}).psi()
+        pbuf, psi = guarded(psi_h.shape)
+        psi.copy_(torch.from_numpy(psi_h))
+        cbuf, c = guarded((w.natoms, w.nbands, plan.nsho))
+        c.zero_()
+        plan.project(psi, c)
+        plan.add(c, psi)
+        tb = plan.tables()
+        plan.project_stored(tb, psi, c)
+        if hasattr(plan, "apply"):
+            D = torch.from_numpy(np.tile(np.eye(plan.nsho), (w.natoms, 1, 1))).cuda()
+            plan.apply(D, psi, c)
+        torch.cuda.synchronize()
+        tb.close()
+        assert intact(pbuf, psi.numel()), "a kernel wrote outside psi"
+        assert intact(cbuf, c.numel()), "a kernel wrote outside coeff"
+        assert bool(torch.isfinite(torch.view_as_real(psi) if w.is_complex else psi).all())
+        assert bool(torch.isfinite(torch.view_as_real(c) if w.is_complex else c).all())
+    finally:
+        plan.close()
+
+
+@pytest.mark.parametrize("k", [4, 5])
+def test_project_and_add_are_bit_reproducible_under_load(sho, k):
+    """Stand-in for racecheck (closed on this pool): both kernels are deterministic by construction (fixed
+    summation order, no atomics), so ANY shared-memory race shows up as a run-to-run difference.  Five runs,
+    half of them with a second stream hammering the GPU to perturb the warp schedule."""
+    import torch
+    w = workloads.make(k, size="small")
+    plan = sho.plan_for(w)
+    psi_h = workloads.Workload(**{**w.__dict__, "psi_dist": "normal"}).psi()
+    c_h = w.coeff(plan.nsho)
+    side = torch.cuda.Stream()
+    junk = torch.randn(2048, 2048, device="cuda")
+    ref = None
+    for it in range(5):
+        if it % 2:
+            with torch.cuda.stream(side):
+                for _ in range(20):
+                    junk = junk @ junk * 1e-3
+        psi = _dev(psi_h)
+        cc = plan.project(psi)
+        out = _dev(psi_h)
+        plan.add(_dev(c_h), out)
+        torch.cuda.synchronize()
+        cur = (cc.clone(), out.clone())
+        if ref is None:
+            ref = cur
+        assert torch.equal(ref[0], cur[0]) and torch.equal(ref[1], cur[1]), "run %d differs bit-wise from run 0" % it
+    plan.close()
+
+
 def test_host_buffer_entry_points(sho):
     w = workloads.make(3, size="small")
     plan = sho.plan_for(w)
