@@ -303,24 +303,28 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
                             }
                     // A predicated-off DMMA still takes its 16 cycles of the pipe (measured), and the compiler
                     // predicates a short "if": enter the unrolled blocks by a jump and leave them by a branch instead.
-#define SHO_ADD_YBLOCK(YT)                                                                              \
+                    // the A fragments of a block are loaded while the MMAs of the block before it issue (two register
+                    // sets take turns; the last block's look-ahead load is harmless: block 8 of the slot is the x block)
+#define SHO_ADD_YBLOCK(YT, CUR, NXT)                                                                    \
     {                                                                                                   \
-        double a_[KQ];                                                                                  \
-        _Pragma("unroll") for (int kk = 0; kk < KQ; ++kk) a_[kk] = fxy[((YT) * KQ + kk) * 32];          \
+        _Pragma("unroll") for (int kk = 0; kk < KQ; ++kk) NXT[kk] = fxy[((YT + 1) * KQ + kk) * 32];     \
         _Pragma("unroll") for (int kk = 0; kk < KQ; ++kk) {                                             \
-            dmma(D[YT][0][0], D[YT][0][1], a_[kk], D1[kk >> 1][0][kk & 1]);                 \
-            dmma(D[YT][1][0], D[YT][1][1], a_[kk], D1[kk >> 1][1][kk & 1]);                 \
+            dmma(D[YT][0][0], D[YT][0][1], CUR[kk], D1[kk >> 1][0][kk & 1]);                            \
+            dmma(D[YT][1][0], D[YT][1][1], CUR[kk], D1[kk >> 1][1][kk & 1]);                            \
         }                                                                                               \
     }
+                    double aA[KQ], aB[KQ];
+#pragma unroll
+                    for (int kk = 0; kk < KQ; ++kk) aA[kk] = aB[kk] = fxy[(ytlo * KQ + kk) * 32];
                     switch (ytlo) {
-                        case 0: SHO_ADD_YBLOCK(0) if (ythi == 0) break;
-                        case 1: SHO_ADD_YBLOCK(1) if (ythi == 1) break;
-                        case 2: SHO_ADD_YBLOCK(2) if (ythi == 2) break;
-                        case 3: SHO_ADD_YBLOCK(3) if (ythi == 3) break;
-                        case 4: SHO_ADD_YBLOCK(4) if (ythi == 4) break;
-                        case 5: SHO_ADD_YBLOCK(5) if (ythi == 5) break;
-                        case 6: SHO_ADD_YBLOCK(6) if (ythi == 6) break;
-                        case 7: SHO_ADD_YBLOCK(7)
+                        case 0: SHO_ADD_YBLOCK(0, aA, aB) if (ythi == 0) break;
+                        case 1: SHO_ADD_YBLOCK(1, aB, aA) if (ythi == 1) break;
+                        case 2: SHO_ADD_YBLOCK(2, aA, aB) if (ythi == 2) break;
+                        case 3: SHO_ADD_YBLOCK(3, aB, aA) if (ythi == 3) break;
+                        case 4: SHO_ADD_YBLOCK(4, aA, aB) if (ythi == 4) break;
+                        case 5: SHO_ADD_YBLOCK(5, aB, aA) if (ythi == 5) break;
+                        case 6: SHO_ADD_YBLOCK(6, aA, aB) if (ythi == 6) break;
+                        case 7: SHO_ADD_YBLOCK(7, aB, aA)
                         default: break;
                     }
 #undef SHO_ADD_YBLOCK

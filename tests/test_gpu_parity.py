@@ -411,11 +411,11 @@ def test_no_write_outside_the_callers_buffers(sho, name):
 
     def guarded(shape):
         n = int(np.prod(shape))
-        buf = torch.full((n + 2 * G,), float("nan"), dtype=tdt, device="cuda")
+        buf = torch.full((n + 2 * G,), complex("nan+nanj") if w.is_complex else float("nan"), dtype=tdt, device="cuda")
         return buf, buf[G:G + n].view(shape)
 
     def intact(buf, n):
-        g = torch.view_as_real(buf) if w.is_complex else buf
+        g = torch.view_as_real(buf).reshape(-1) if w.is_complex else buf
         k = 2 if w.is_complex else 1
         return bool(torch.isnan(g[:G * k]).all()) and bool(torch.isnan(g[(G + n) * k:]).all())
 
