@@ -45,6 +45,20 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0}, "fallback"
 
 
+def committed_traffic(workload, dtype, kernel):
+    """dram__bytes_read + dram__bytes_write of one launch from the committed ncu --set full capture of this
+    workload and kernel (profiles/traffic.json, written from the .ncu-rep named there), or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(path):
+        return None, None
+    with open(path) as f:
+        t = json.load(f)
+    e = t.get("%s/%s/%s" % (workload, dtype, kernel))
+    if not e:
+        return None, None
+    return float(e["dram_bytes_read"]) + float(e["dram_bytes_write"]), "profiles/traffic.json <- %s" % e.get("source", "?")
+
+
 def geometry(w, boxes=None):
     """Counts only (no method arithmetic): box points and algorithmic flops of one project (= one add)
     launch over all atoms and bands.  F = 2 P [ box M + n_z n_x pairs + n_z N_SHO ] per atom and band
@@ -116,23 +130,31 @@ class ClockSampler:
 
 def oracle_sample_setup(w, cpu_seconds=20.0):
     """A bounded sample of the workload for the oracle: the first n_a atoms x n_b bands, sized for about
-    ``cpu_seconds`` core-seconds (project + add)."""
+    ``cpu_seconds`` core-seconds (project + add).  The oracle's speed is calibrated on one atom first, so the
+    sample runs at least 2 s of wall time on any host."""
     import oracle
     cores = oracle.num_threads()
     g = geometry(w)
     n_b = min(w.nbands, cores)
-    rate = (2.5e8 if w.is_complex else 5.0e8)                 # rough oracle speed, box-point*coefficients / s / core
-    t_pair = 2.0 * float(np.mean(g["box_points"])) * g["nsho"] / rate
-    n_a = int(max(1, min(w.natoms, round(cpu_seconds / max(t_pair * n_b, 1e-9)))))
     psi = w.psi(range(n_b))
     if w.psi_dist == "zero":
         psi = workloads.Workload(**{**w.__dict__, "psi_dist": "normal"}).psi(range(n_b))
     wide = np.complex128 if w.is_complex else np.float64
     psi = psi.astype(wide)
+    t_atom = 1e9
+    for _ in range(2):                                             # the first call also loads the library and starts OpenMP
+        t0 = time.perf_counter()
+        c1 = oracle.project(w.ng, w.h, w.periodic, w.kfrac, w.pos[:1], w.sigma[:1], w.numax, psi, w.rcut_sigma)
+        oracle.add(w.ng, w.h, w.periodic, w.kfrac, w.pos[:1], w.sigma[:1], w.numax, c1, psi, w.rcut_sigma)
+        t_atom = min(t_atom, max(time.perf_counter() - t0, 1e-4))
+    t_atom *= float(np.mean(g["box_points"])) / max(float(g["box_points"][0]), 1.0)
+    wall = max(3.5, cpu_seconds / max(cores, 1))                   # seconds of wall time to aim for (>= 2 s, SURVEY 8(d))
+    n_a = int(max(1, min(w.natoms, round(wall / t_atom))))
     sub_box = int(g["box_points"][:n_a].sum()) * n_b
     return {"n_a": n_a, "n_b": n_b, "psi": psi, "cores": cores, "box_band_points": sub_box,
-            "bytes": 3.0 * sub_box * ESZ[w.dtype],
-            "sample": "first %d atoms x %d bands of %s: oracle project (direct triple sum) then oracle add" % (n_a, n_b, w.name)}
+            "bytes": 3.0 * sub_box * ESZ[w.dtype], "pairs": n_a * n_b,
+            "sample": "first %d atoms x %d bands of %s = %d (atom, band) pairs: oracle project (direct triple sum) then oracle add"
+                      % (n_a, n_b, w.name, n_a * n_b)}
 
 
 def oracle_sample_run(w, s):
@@ -170,11 +192,54 @@ def run_reference(args, w):
 # --------------------------------------------------------------------------------------------------
 
 
+def stored_vs_on_the_fly(sho, torch, dev, w3, steps):
+    """On-the-fly projection against the stored-projector baseline (a7) on one workload: median device times, table
+    bytes, and the baseline's own bound max(table bytes / HBM, its flops / FP64 peak)."""
+    plan = sho.plan_for(w3)
+    g3 = geometry(w3, plan.boxes())
+    tdt = {"r64": torch.float64, "c128": torch.complex128, "r32": torch.float32, "c64": torch.complex64}[w3.dtype]
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(w3.seed)
+    psi = torch.randn((w3.nbands, w3.ng[2], w3.ng[1], w3.ng[0]), dtype=tdt, device=dev, generator=gen)
+    coeff = plan.new_coeff(w3.nbands, dev)
+    stream = torch.cuda.current_stream()
+    need = plan.tables_bytes()
+    out = {"workload": w3.name, "table_bytes": need}
+    if need > 0.8 * torch.cuda.mem_get_info(dev)[0]:
+        out["status"] = "does not fit"
+        plan.close()
+        return out
+    tb = plan.tables()
+
+    def med(fn):
+        for _ in range(2):
+            fn()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(max(steps, 3))]
+        for a, b in evs:
+            a.record(stream); fn(); b.record(stream)
+        torch.cuda.synchronize()
+        return float(np.median([a.elapsed_time(b) for a, b in evs])) * 1e-3
+
+    t_fly = med(lambda: plan.project(psi, coeff, stream))
+    t_sto = med(lambda: plan.project_stored(tb, psi, coeff, stream))
+    tb.close()
+    plan.close()
+    peaks, _ = measured_peaks()
+    P = g3["P"]
+    f_sto = 2.0 * P * g3["nsho"] * float(g3["sum_box"]) * w3.nbands       # non-separable: N_SHO MACs per box point and band
+    bound = max(need / (peaks["hbm_gbs"] * 1e9), f_sto / (FP64_PEAK_TFLOPS * 1e12))
+    out.update(status="ok", ms_project_on_the_fly=1e3 * t_fly, ms_project_stored=1e3 * t_sto, slowdown_vs_on_the_fly=t_sto / t_fly,
+               table_gbs=need / t_sto / 1e9, stored_bound_ms=1e3 * bound, stored_frac_of_its_bound=bound / t_sto,
+               on_the_fly_gain_if_stored_ran_at_its_bound=bound / t_fly)
+    return out
+
+
 def run_ours(args, w):
     import torch
     import torch.distributed as dist
 
     import paper_1905_00480_b200 as sho
+    from paper_1905_00480_b200 import sharding
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -192,9 +257,12 @@ def run_ours(args, w):
     g = geometry(w, plan.boxes())
     nb, esz, P = w.nbands, ESZ[w.dtype], g["P"]
     tdt = {"r64": torch.float64, "c128": torch.complex128, "r32": torch.float32, "c64": torch.complex64}[w.dtype]
-    # weak scaling over bands: every rank owns nbands bands of its own, seeded per rank
+    # weak scaling over bands: the job has world * nbands bands, rank r owns the contiguous
+    # range sharding.band_range gives it and draws its psi from a seed of its own; no data-path collective
+    band_lo, band_hi = sharding.band_range(world * nb, rank, world)
+    assert band_hi - band_lo == nb
     gen = torch.Generator(device=dev)
-    gen.manual_seed(w.seed * 1000 + rank)
+    gen.manual_seed(w.seed * 1000 + band_lo)
     shape = (nb, w.ng[2], w.ng[1], w.ng[0])
     psi = torch.randn(shape, dtype=tdt, device=dev, generator=gen)   # read by project
     psi_out = torch.zeros(shape, dtype=tdt, device=dev)             # accumulated into by add (stays finite)
@@ -225,12 +293,10 @@ def run_ours(args, w):
     barrier()
     clocks = sampler.stop() if sampler else None
     t_total = ev[0][0].elapsed_time(ev[-1][2]) * 1e-3
-    t_prj = float(np.mean([e[0].elapsed_time(e[1]) for e in ev])) * 1e-3
-    t_add = float(np.mean([e[1].elapsed_time(e[2]) for e in ev])) * 1e-3
-    if world > 1:
-        tt = torch.tensor([t_total, t_prj, t_add], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_total, t_prj, t_add = (float(x) for x in tt.cpu())
+    # per-kernel times: median over the timed steps (the paper's protocol)
+    t_prj = float(np.median([e[0].elapsed_time(e[1]) for e in ev])) * 1e-3
+    t_add = float(np.median([e[1].elapsed_time(e[2]) for e in ev])) * 1e-3
+    t_total, t_prj, t_add = sharding.max_over_ranks([t_total, t_prj, t_add], device=dev)
 
     box_bytes = float(g["sum_box"]) * nb * esz                        # B_box of one rank
     step_bytes = 3.0 * box_bytes * world
@@ -239,40 +305,49 @@ def run_ours(args, w):
     F = g["flops_per_band"] * nb                                     # algorithmic flops of one project (= one add) launch
     dom, t_dom = ("sho_add_kernel", t_add) if t_add >= t_prj else ("sho_project_kernel", t_prj)
     alu_peak = FP64_PEAK_TFLOPS                                      # arithmetic is fp64 for all four dtypes
-    # dram__bytes_read + dram__bytes_write of one launch from the committed ncu --set full capture (cfg5 only)
-    traffic = {"sho_add_kernel": 8.283107e9 + 7.196529e9, "sho_project_kernel": 9.560539e9 + 0.262074e9}.get(dom) \
-        if (w.name == "cfg5" and w.dtype == "c128") else None
+    traffic, traffic_src = committed_traffic(w.name, w.dtype, dom)
     roofline = {"bound": "alu", "kernel": dom, "achieved": F / t_dom / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
-                "frac": F / t_dom / 1e12 / alu_peak, "traffic": traffic,
-                "traffic_source": "profiles/r1_final_cfg5_ncu_full.txt (bytes per launch)" if traffic else None,
+                "frac": F / t_dom / 1e12 / alu_peak, "traffic": traffic, "traffic_source": traffic_src,
                 "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md); DMMA/DFMA micro-benchmark in fp64_peak_measured_tflops",
-                "flops_per_launch": F}
+                "flops_per_launch": F,
+                "frac_project": F / t_prj / 1e12 / alu_peak, "frac_add": F / t_add / 1e12 / alu_peak}
 
-    # ---- end to end through the HOST-buffer C-ABI calls (pinned host memory) ----
+    # ---- the three-step action project -> D -> add in one call (f2), device resident, outside the timed region ----
+    dmat = torch.from_numpy(w.dmatrix(plan.nsho)).to(dev)
+    plan.apply(dmat, psi_out, coeff, stream)
+    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    e0.record(stream)
+    plan.dmul(dmat, coeff, coeff, stream)
+    e1.record(stream)
+    plan.apply(dmat, psi_out, coeff, stream)
+    e2.record(stream)
+    torch.cuda.synchronize()
+    t_dmul, t_apply = e0.elapsed_time(e1) * 1e-3, e1.elapsed_time(e2) * 1e-3
+    psi_out.zero_()
+
+    # ---- end to end through the HOST-buffer C-ABI call sho_apply_host (pinned host memory): psi is uploaded once,
+    # project -> D -> add run on the device, psi is downloaded once; the coefficients never leave the device ----
     e2e = None
     if not args.no_e2e:
         hp = torch.empty(shape, dtype=tdt, pin_memory=True)
-        hc = torch.empty((w.natoms, nb, plan.nsho), dtype=tdt, pin_memory=True)
+        hd = torch.from_numpy(w.dmatrix(plan.nsho)).pin_memory()
         hp.copy_(psi)
         torch.cuda.synchronize()
         ke = max(1, min(args.steps, args.e2e_steps))
-        plan.project_host(hp, hc, stream); plan.add_host(hc, hp, stream)      # warm-up (allocates the plan workspace)
+        plan.apply_host(hd, hp, stream)                                  # warm-up (allocates the plan workspace)
         hp.copy_(psi)
         barrier()
         t0 = time.perf_counter()
         for _ in range(ke):
-            plan.project_host(hp, hc, stream)
-            plan.add_host(hc, hp, stream)
+            plan.apply_host(hd, hp, stream)
         torch.cuda.synchronize()
         te = time.perf_counter() - t0
-        if world > 1:
-            tt = torch.tensor([te], dtype=torch.float64, device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            te = float(tt.cpu()[0])
-        psi_b, c_b = int(np.prod(shape)) * esz, w.natoms * nb * plan.nsho * esz
-        e2e = {"value": step_bytes * ke / te / 1e9, "unit": "GB/s", "h2d_bytes_per_step": 2 * psi_b + c_b,
-               "d2h_bytes_per_step": psi_b + c_b, "steps": ke, "ms_per_step": 1e3 * te / ke}
-        del hp, hc
+        (te,) = sharding.max_over_ranks([te], device=dev)
+        psi_b, d_b = int(np.prod(shape)) * esz, w.natoms * plan.nsho * plan.nsho * 8
+        e2e = {"value": step_bytes * ke / te / 1e9, "unit": "GB/s", "h2d_bytes_per_step": psi_b + d_b,
+               "d2h_bytes_per_step": psi_b, "steps": ke, "ms_per_step": 1e3 * te / ke,
+               "call": "sho_apply_host (project -> D c -> add, one upload and one download of psi per step)"}
+        del hp, hd
 
     if rank != 0:
         if world > 1:
@@ -306,6 +381,13 @@ def run_ours(args, w):
             stored.update(status="ok", ms_project_stored=1e3 * t_sto, table_gbs=need / t_sto / 1e9,
                           slowdown_vs_on_the_fly=t_sto / t_prj,
                           table_bytes_over_psi_box_bytes=need / box_bytes)
+    # cfg 3 is the config BASELINE.json states the on-the-fly vs stored comparison on; when the benched workload's tables do
+    # not fit, run that comparison as a sub-leg (outside the timed region) so that it is observed in the default run too
+    stored_cfg3 = None
+    if not args.no_stored and w.name != "cfg3" and world == 1:
+        del psi_out
+        torch.cuda.empty_cache()
+        stored_cfg3 = stored_vs_on_the_fly(sho, torch, dev, workloads.make(3), min(args.steps, 5))
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         s = oracle_sample_setup(w, cpu_seconds=args.ref_cpu_seconds)
@@ -324,11 +406,16 @@ def run_ours(args, w):
         "detail": {
             "ms_project": 1e3 * t_prj, "ms_add": 1e3 * t_add,
             "psi_gbs_box_project": box_bytes / t_prj / 1e9, "psi_gbs_box_add": 2 * box_bytes / t_add / 1e9,
-            "frac_hbm_peak_project": box_bytes / t_prj / 1e9 / peaks["hbm_gbs"], "frac_hbm_peak_add": 2 * box_bytes / t_add / 1e9 / peaks["hbm_gbs"],
-            "frac_hbm_peak_step": value / world / peaks["hbm_gbs"], "hbm_peak_gbs": peaks["hbm_gbs"], "hbm_peak_kind": peak_kind,
+            "box_bytes_over_hbm_peak_project": box_bytes / t_prj / 1e9 / peaks["hbm_gbs"],
+            "box_bytes_over_hbm_peak_add": 2 * box_bytes / t_add / 1e9 / peaks["hbm_gbs"],
+            "box_bytes_over_hbm_peak_step": value / world / peaks["hbm_gbs"],
+            "box_bytes_note": "psi-GB/s(box) counts every psi value once per box that holds it (the traffic of a kernel without reuse, "
+                              "BASELINE.json's metric); these ratios exceed 1 when L2 / ownership tiling capture the overlap and are "
+                              "NOT an HBM roofline -- see roofline (FP64 pipe) and roofline.traffic (real DRAM bytes)", "hbm_peak_gbs": peaks["hbm_gbs"], "hbm_peak_kind": peak_kind,
             "atom_band_per_s": world * info["atoms_nonempty"] * nb * args.steps / t_total,
             "tflops_project": F / t_prj / 1e12, "tflops_add": F / t_add / 1e12, "fp64_peak_measured_tflops": fp64_meas,
-            "stored_baseline": stored, "sum_box_points": g["sum_box"], "psi_bytes_unique": int(np.prod(shape)) * esz, "add_tile_pairs": info["add_pairs"],
+            "ms_dmul": 1e3 * t_dmul, "ms_apply_project_dmul_add": 1e3 * t_apply,
+            "stored_baseline": stored, "stored_baseline_cfg3": stored_cfg3, "sum_box_points": g["sum_box"], "psi_bytes_unique": int(np.prod(shape)) * esz, "add_tile_pairs": info["add_pairs"],
         },
     }
     print(json.dumps(line))

@@ -122,18 +122,41 @@ sho_status sho_project_stored(const sho_plan* plan, const sho_tables* tables, co
                               void* coeff, void* cuda_stream);
 
 /*
+ * Step (2) of the non-local action: d[a][b][i] = sum_j D[a][i][j] c[a][b][j], with the atomic
+ * matrix in the SHO representation (eq. (27)-(28): "a real-valued matrix of dimension
+ * N_SHO").  dmat DEVICE fp64 [natoms][N_SHO][N_SHO] row-major (D[a][i][j]; need not be symmetric), coeff_in
+ * and coeff_out DEVICE [natoms][nbands][N_SHO] in the plan's dtype; coeff_out may be the same buffer as
+ * coeff_in.  Asynchronous on the stream, allocates nothing.
+ */
+sho_status sho_dmul(const sho_plan* plan, const double* dmat, const void* coeff_in, int32_t nbands, void* coeff_out,
+                    void* cuda_stream);
+
+/*
+ * The three steps of PAPER.md:187-190 in one call: c = project(psi); d = D c; psi += add(d), on one stream.
+ * psi DEVICE in/out, coeff_work DEVICE [natoms][nbands][N_SHO] caller-owned scratch (holds d on return).
+ */
+sho_status sho_apply(const sho_plan* plan, const double* dmat, void* psi, int32_t nbands, void* coeff_work,
+                     void* cuda_stream);
+
+/*
  * End-to-end variants with HOST buffers (pinned or pageable): copy in, run the same kernels, copy
  * out, and synchronise the stream before returning.  They use a device workspace owned by the plan
- * that is grown on demand (the only hot-path calls that may allocate).  The bands are independent
- * (eq. (25)), so the calls work in chunks of bands (about 512 MB of psi each; environment
- * variable SHO_HOST_CHUNK_BANDS overrides the chunk size) and overlap the H2D copy of the next chunk,
- * the kernel of this one and the D2H copy of the previous one on two copy streams owned by the plan;
- * all of it is ordered after the work already queued on cuda_stream.
+ * (the only hot-path calls that may allocate; it is grown on demand and bounded by the chunk size, not
+ * by nbands).  The bands are independent (eq. (25)), so the calls work in chunks of bands
+ * (about 512 MB of psi each; environment variable SHO_HOST_CHUNK_BANDS overrides the chunk size)
+ * through a ring of three chunk buffers and overlap the H2D copy of the next chunk, the kernels of this
+ * one and the D2H copy of the previous one on two copy streams owned by the plan; all of it is ordered
+ * after the work already queued on cuda_stream.  If a step fails mid-way the call waits for everything
+ * it has queued before it returns the error.
  *   sho_project_host: psi HOST (read), coeff HOST (written)
  *   sho_add_host:     coeff HOST (read), psi HOST (in/out)
+ *   sho_apply_host:   dmat HOST fp64 [natoms][N_SHO][N_SHO], psi HOST (in/out): psi is uploaded ONCE,
+ *                     project -> D -> add run on the device, psi is downloaded once; the coefficients
+ *                     never leave the device
  */
 sho_status sho_project_host(sho_plan* plan, const void* psi_host, int32_t nbands, void* coeff_host, void* cuda_stream);
 sho_status sho_add_host(sho_plan* plan, const void* coeff_host, int32_t nbands, void* psi_host, void* cuda_stream);
+sho_status sho_apply_host(sho_plan* plan, const double* dmat_host, void* psi_host, int32_t nbands, void* cuda_stream);
 
 /* FP64 FMA-pipe micro-benchmark used by bench.py for the roofline denominator: runs `iters` rounds of
  * eight independent DFMA chains per thread on every SM and returns the achieved FLOP/s in *flops_per_s

@@ -85,6 +85,9 @@ def lib():
     L.sho_project_host.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
     L.sho_add_host.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
     L.sho_measure_fp64_peak.argtypes = [C.c_int32, _f64p]
+    L.sho_dmul.argtypes = [_vp, _vp, _vp, C.c_int32, _vp, _vp]
+    L.sho_apply.argtypes = [_vp, _vp, _vp, C.c_int32, _vp, _vp]
+    L.sho_apply_host.argtypes = [_vp, _vp, _vp, C.c_int32, _vp]
     for name in DECLARED_SYMBOLS:
         fn = getattr(L, name)   # AttributeError here = header and library disagree
         if name not in ("sho_status_string", "sho_last_error"):
@@ -167,6 +170,7 @@ class Plan:
         self._h = None
         _check(st, "sho_plan_create")
         self._h = h_
+        self.device = _torch().cuda.current_device()      # the plan belongs to the device that was current (sho.h)
 
     # -- housekeeping ---------------------------------------------------------------------------
     def close(self):
@@ -208,6 +212,8 @@ class Plan:
         torch = _torch()
         if not (isinstance(psi, torch.Tensor) and psi.is_cuda and psi.is_contiguous()):
             raise ValueError("%s: psi must be a contiguous CUDA tensor" % where)
+        if psi.device.index != self.device:
+            raise ValueError("%s: psi lives on cuda:%s, the plan on cuda:%d" % (where, psi.device.index, self.device))
         if psi.dtype != _torch_dtype(self.dtype):
             raise ValueError("%s: psi dtype %s does not match the plan (%s)" % (where, psi.dtype, self.dtype))
         if psi.dim() != 4 or tuple(psi.shape[1:]) != (self.ng[2], self.ng[1], self.ng[0]):
@@ -218,6 +224,8 @@ class Plan:
         torch = _torch()
         if not (isinstance(coeff, torch.Tensor) and coeff.is_cuda and coeff.is_contiguous()):
             raise ValueError("%s: coeff must be a contiguous CUDA tensor" % where)
+        if coeff.device.index != self.device:
+            raise ValueError("%s: coeff lives on cuda:%s, the plan on cuda:%d" % (where, coeff.device.index, self.device))
         if coeff.dtype != _torch_dtype(self.dtype) or tuple(coeff.shape) != (self.natoms, nb, self.nsho):
             raise ValueError("%s: coeff must be [natoms][nbands][N_SHO] of the plan's dtype" % where)
 
@@ -239,6 +247,34 @@ class Plan:
         nb = self._check_psi(psi, "sho_add")
         self._check_coeff(coeff, nb, "sho_add")
         _check(lib().sho_add(self._h, coeff.data_ptr(), nb, psi.data_ptr(), _stream_handle(stream)), "sho_add")
+        return psi
+
+    def _check_dmat(self, dmat, where):
+        torch = _torch()
+        if not (isinstance(dmat, torch.Tensor) and dmat.is_cuda and dmat.is_contiguous() and dmat.dtype == torch.float64
+                and tuple(dmat.shape) == (self.natoms, self.nsho, self.nsho) and dmat.device.index == self.device):
+            raise ValueError("%s: dmat must be a contiguous float64 CUDA tensor [natoms][N_SHO][N_SHO] on the plan's device" % where)
+
+    def dmul(self, dmat, coeff, out=None, stream=None):
+        """Step (2): out[a][b][i] = sum_j dmat[a][i][j] coeff[a][b][j] (out may be coeff itself)."""
+        nb = int(coeff.shape[1])
+        self._check_coeff(coeff, nb, "sho_dmul")
+        self._check_dmat(dmat, "sho_dmul")
+        if out is None:
+            out = self.new_coeff(nb, coeff.device)
+        self._check_coeff(out, nb, "sho_dmul")
+        _check(lib().sho_dmul(self._h, dmat.data_ptr(), coeff.data_ptr(), nb, out.data_ptr(), _stream_handle(stream)), "sho_dmul")
+        return out
+
+    def apply(self, dmat, psi, coeff_work=None, stream=None):
+        """psi += add(dmat * project(psi)): the three steps of the non-local action on one stream."""
+        nb = self._check_psi(psi, "sho_apply")
+        self._check_dmat(dmat, "sho_apply")
+        if coeff_work is None:
+            coeff_work = self.new_coeff(nb, psi.device)
+        self._check_coeff(coeff_work, nb, "sho_apply")
+        _check(lib().sho_apply(self._h, dmat.data_ptr(), psi.data_ptr(), nb, coeff_work.data_ptr(), _stream_handle(stream)),
+               "sho_apply")
         return psi
 
     def tables_bytes(self) -> int:
@@ -280,6 +316,23 @@ class Plan:
         _check(lib().sho_project_host(self._h, pp, nb, cp, _stream_handle(stream)), "sho_project_host")
         return coeff_host
 
+    def apply_host(self, dmat_host, psi_host, stream=None):
+        nb = int(psi_host.shape[0])
+        pp = self._host_ptr(psi_host, (nb, self.ng[2], self.ng[1], self.ng[0]), "sho_apply_host")
+        torch = _torch()
+        shape = (self.natoms, self.nsho, self.nsho)
+        if isinstance(dmat_host, torch.Tensor):
+            if dmat_host.is_cuda or not dmat_host.is_contiguous() or dmat_host.dtype != torch.float64 or tuple(dmat_host.shape) != shape:
+                raise ValueError("sho_apply_host: dmat must be a contiguous float64 host tensor [natoms][N_SHO][N_SHO]")
+            dp = dmat_host.data_ptr()
+        else:
+            if not (isinstance(dmat_host, np.ndarray) and dmat_host.flags.c_contiguous and dmat_host.dtype == np.float64
+                    and dmat_host.shape == shape):
+                raise ValueError("sho_apply_host: dmat must be a C-contiguous float64 array [natoms][N_SHO][N_SHO]")
+            dp = dmat_host.ctypes.data
+        _check(lib().sho_apply_host(self._h, dp, pp, nb, _stream_handle(stream)), "sho_apply_host")
+        return psi_host
+
     def add_host(self, coeff_host, psi_host, stream=None):
         nb = int(psi_host.shape[0])
         pp = self._host_ptr(psi_host, (nb, self.ng[2], self.ng[1], self.ng[0]), "sho_add_host")
@@ -299,6 +352,18 @@ def sho_add(plan: Plan, coeff, psi, stream=None):
 
 def sho_project_stored(plan: Plan, tables: Tables, psi, coeff=None, stream=None):
     return plan.project_stored(tables, psi, coeff, stream)
+
+
+def sho_dmul(plan: Plan, dmat, coeff, out=None, stream=None):
+    return plan.dmul(dmat, coeff, out, stream)
+
+
+def sho_apply(plan: Plan, dmat, psi, coeff_work=None, stream=None):
+    return plan.apply(dmat, psi, coeff_work, stream)
+
+
+def sho_apply_host(plan: Plan, dmat_host, psi_host, stream=None):
+    return plan.apply_host(dmat_host, psi_host, stream)
 
 
 def sho_project_host(plan: Plan, psi_host, coeff_host, stream=None):

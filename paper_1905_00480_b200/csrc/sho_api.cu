@@ -55,13 +55,13 @@ static void plan_free_device(sho_plan* p)
 {
     cudaFree(p->d_atoms); cudaFree(p->d_order); cudaFree(p->d_nxyz);
     cudaFree(p->d_tile_ptr); cudaFree(p->d_tile_ent); cudaFree(p->d_tile_list); cudaFree(p->d_tile_info); cudaFree(p->d_cainv); cudaFree(p->d_t2pos); cudaFree(p->d_cidx);
-    cudaFree(p->ws_psi); cudaFree(p->ws_c);
+    cudaFree(p->ws_psi); cudaFree(p->ws_c); cudaFree(p->ws_d);
     if (p->s_in) cudaStreamDestroy(p->s_in);
     if (p->s_out) cudaStreamDestroy(p->s_out);
     p->s_in = nullptr; p->s_out = nullptr;
     p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr; p->d_cidx = nullptr;
     p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr; p->d_tile_info = nullptr;
-    p->ws_psi = nullptr; p->ws_c = nullptr;
+    p->ws_psi = nullptr; p->ws_c = nullptr; p->ws_d = nullptr;
 }
 
 }  // namespace sho
@@ -128,7 +128,7 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
     if (!p) { set_error("sho_plan_create: host allocation failed"); return SHO_ERR_OOM; }
     p->d_atoms = nullptr; p->d_order = nullptr; p->d_nxyz = nullptr;
     p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr; p->d_tile_info = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr; p->d_cidx = nullptr;
-    p->ws_psi = nullptr; p->ws_c = nullptr; p->ws_psi_bytes = 0; p->ws_c_bytes = 0;
+    p->ws_psi = nullptr; p->ws_c = nullptr; p->ws_d = nullptr; p->ws_psi_bytes = 0; p->ws_c_bytes = 0; p->ws_d_bytes = 0;
     p->s_in = nullptr; p->s_out = nullptr;
     p->rcut_sigma = rcut_sigma;
     p->dtype = dtype;
@@ -483,6 +483,30 @@ sho_status sho_project_stored(const sho_plan* plan, const sho_tables* tables, co
     return launch_project_stored(plan, tables, psi, nbands, coeff, static_cast<cudaStream_t>(cuda_stream));
 }
 
+// ---- step (2) and the three-step non-local action ------------------------------------------------
+sho_status sho_dmul(const sho_plan* plan, const double* dmat, const void* coeff_in, int32_t nbands, void* coeff_out,
+                    void* cuda_stream)
+{
+    if (plan && plan->g.natoms == 0 && nbands > 0) return SHO_OK;
+    sho_status st = check_hot("sho_dmul", plan, coeff_in, coeff_out, nbands);
+    if (st != SHO_OK) return st;
+    if (!dmat) { set_error("sho_dmul: null argument"); return SHO_ERR_INVALID_ARG; }
+    return launch_dmul(plan, dmat, coeff_in, nbands, coeff_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+sho_status sho_apply(const sho_plan* plan, const double* dmat, void* psi, int32_t nbands, void* coeff_work, void* cuda_stream)
+{
+    if (plan && plan->g.natoms == 0 && psi && nbands > 0) return SHO_OK;
+    sho_status st = check_hot("sho_apply", plan, psi, coeff_work, nbands);
+    if (st != SHO_OK) return st;
+    if (!dmat) { set_error("sho_apply: null argument"); return SHO_ERR_INVALID_ARG; }
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    if ((st = launch_project(plan, psi, nbands, coeff_work, s)) != SHO_OK) return st;
+    if ((st = launch_dmul(plan, dmat, coeff_work, nbands, coeff_work, s)) != SHO_OK) return st;
+    if (plan->n_tile_list == 0) return SHO_OK;
+    return launch_add(plan, coeff_work, nbands, psi, s);
+}
+
 // ---- HOST-buffer end-to-end variants ------------------------------------------------------------
 static sho_status ws_reserve(void** ws, size_t* have, size_t need, const char* what)
 {
@@ -492,40 +516,6 @@ static sho_status ws_reserve(void** ws, size_t* have, size_t need, const char* w
     cudaError_t e = cudaMalloc(ws, need);
     if (e != cudaSuccess) { cudaGetLastError(); set_error("%s: cannot allocate %zu bytes of device workspace", what, need); return SHO_ERR_OOM; }
     *have = need;
-    return SHO_OK;
-}
-
-// The bands are independent, so the host-buffer calls pipeline them in chunks: the H2D copy of chunk i+1, the
-// kernel of chunk i and the D2H copy of chunk i-1 run at the same time on three streams (PCIe is full duplex).
-// A chunk's coefficients [natoms][chunk][N_SHO] are a 2D sub-array of the caller's [natoms][nbands][N_SHO].
-struct HostPipe {
-    cudaStream_t s, s_in, s_out;
-    std::vector<cudaEvent_t> ev;
-    cudaEvent_t event()
-    {
-        cudaEvent_t e = nullptr;
-        cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
-        ev.push_back(e);
-        return e;
-    }
-    void after(cudaStream_t waiter, cudaStream_t signaller)      // waiter continues after what signaller has queued
-    {
-        cudaEvent_t e = event();
-        cudaEventRecord(e, signaller);
-        cudaStreamWaitEvent(waiter, e, 0);
-    }
-    ~HostPipe() { for (cudaEvent_t e : ev) cudaEventDestroy(e); }
-};
-
-static sho_status host_pipe_open(sho_plan* plan, cudaStream_t s, HostPipe* hp, const char* what)
-{
-    if (!plan->s_in && cudaStreamCreateWithFlags(&plan->s_in, cudaStreamNonBlocking) != cudaSuccess)
-        return cuda_fail(cudaGetLastError(), what);
-    if (!plan->s_out && cudaStreamCreateWithFlags(&plan->s_out, cudaStreamNonBlocking) != cudaSuccess)
-        return cuda_fail(cudaGetLastError(), what);
-    hp->s = s; hp->s_in = plan->s_in; hp->s_out = plan->s_out;
-    hp->after(hp->s_in, s);                 // the copies start after what the caller queued on its stream
-    hp->after(hp->s_out, s);
     return SHO_OK;
 }
 
@@ -543,86 +533,122 @@ static int host_chunk_bands(const sho_plan* plan, int nbands)
     return std::min(cb, nbands);
 }
 
+// The bands are independent, so the host-buffer calls pipeline them in chunks through a ring of kHostRing chunk
+// buffers on the device (the workspace is bounded by the chunk size, not by nbands): the H2D copy of chunk i+1, the
+// kernels of chunk i and the D2H copy of chunk i-1 run at the same time on three streams (PCIe is full duplex).  A
+// ring slot is reused only after the D2H copy (hence the kernels) of the chunk that used it last has finished.  A
+// chunk's coefficients [natoms][chunk][N_SHO] are a 2D sub-array of the caller's [natoms][nbands][N_SHO].
+constexpr int kHostRing = 3;
+enum HostMode { kHostProject, kHostAdd, kHostApply };
+
+static sho_status host_run(sho_plan* plan, HostMode mode, const char* fn, void* psi_host, void* coeff_host,
+                           const double* dmat_dev, int32_t nbands, cudaStream_t s)
+{
+    const size_t esz = elem_size(plan->dtype);
+    const size_t band_bytes = (size_t)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * esz;
+    const size_t row_bytes = (size_t)plan->g.nsho * esz;                     // coefficients of one (atom, band)
+    const int cb = host_chunk_bands(plan, nbands);
+    const int nchunks = (nbands + cb - 1) / cb;
+    const int nring = std::min(nchunks, kHostRing);
+    const size_t psi_slot = band_bytes * cb, c_slot = std::max<size_t>((size_t)plan->g.natoms * cb * row_bytes, 16);
+    sho_status st;
+    if ((st = ws_reserve(&plan->ws_psi, &plan->ws_psi_bytes, psi_slot * nring, fn)) != SHO_OK) return st;
+    if ((st = ws_reserve(&plan->ws_c, &plan->ws_c_bytes, c_slot * nring, fn)) != SHO_OK) return st;
+    if (!plan->s_in && cudaStreamCreateWithFlags(&plan->s_in, cudaStreamNonBlocking) != cudaSuccess) return cuda_fail(cudaGetLastError(), fn);
+    if (!plan->s_out && cudaStreamCreateWithFlags(&plan->s_out, cudaStreamNonBlocking) != cudaSuccess) return cuda_fail(cudaGetLastError(), fn);
+    cudaStream_t s_in = plan->s_in, s_out = plan->s_out;
+    std::vector<cudaEvent_t> events;
+    auto mark = [&](cudaStream_t signaller) -> cudaEvent_t {                            // an event behind what signaller has queued
+        cudaEvent_t e = nullptr;
+        cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+        events.push_back(e);
+        cudaEventRecord(e, signaller);
+        return e;
+    };
+    // waiter continues after what signaller has queued (the caller's stream may be the default stream, handle 0)
+    auto after = [&](cudaStream_t waiter, cudaStream_t signaller) { cudaStreamWaitEvent(waiter, mark(signaller), 0); };
+    // on any failure: let everything that was queued finish before the caller gets its buffers back
+    auto finish = [&](sho_status status) {
+        cudaStreamSynchronize(s_in); cudaStreamSynchronize(s); cudaStreamSynchronize(s_out);
+        for (cudaEvent_t e : events) cudaEventDestroy(e);
+        return status;
+    };
+    after(s_in, s);                         // the copies start after what the caller queued on its stream
+    after(s_out, s);
+    cudaEvent_t slot_free[kHostRing] = { nullptr, nullptr, nullptr };
+    cudaError_t e = cudaSuccess;
+    for (int i = 0, b0 = 0; b0 < nbands; ++i, b0 += cb) {
+        const int nb = std::min(cb, nbands - b0), slot = i % nring;
+        char* d_psi = static_cast<char*>(plan->ws_psi) + (size_t)slot * psi_slot;
+        char* d_c = static_cast<char*>(plan->ws_c) + (size_t)slot * c_slot;                 // [natoms][nb][N_SHO]
+        char* h_psi = static_cast<char*>(psi_host) + (size_t)b0 * band_bytes;
+        char* h_c = coeff_host ? static_cast<char*>(coeff_host) + (size_t)b0 * row_bytes : nullptr;
+        if (slot_free[slot]) cudaStreamWaitEvent(s_in, slot_free[slot], 0);
+        if (mode == kHostAdd && plan->g.natoms > 0) {
+            e = cudaMemcpy2DAsync(d_c, (size_t)nb * row_bytes, h_c, (size_t)nbands * row_bytes, (size_t)nb * row_bytes,
+                                  (size_t)plan->g.natoms, cudaMemcpyHostToDevice, s_in);
+            if (e != cudaSuccess) return finish(cuda_fail(e, fn));
+        }
+        e = cudaMemcpyAsync(d_psi, h_psi, band_bytes * nb, cudaMemcpyHostToDevice, s_in);
+        if (e != cudaSuccess) return finish(cuda_fail(e, fn));
+        after(s, s_in);
+        if (plan->g.natoms > 0) {
+            if (mode == kHostProject) st = launch_project(plan, d_psi, nb, d_c, s);
+            else if (mode == kHostAdd) st = plan->n_tile_list ? launch_add(plan, d_c, nb, d_psi, s) : SHO_OK;
+            else {
+                st = launch_project(plan, d_psi, nb, d_c, s);
+                if (st == SHO_OK) st = launch_dmul(plan, dmat_dev, d_c, nb, d_c, s);
+                if (st == SHO_OK && plan->n_tile_list) st = launch_add(plan, d_c, nb, d_psi, s);
+            }
+            if (st != SHO_OK) return finish(st);
+        }
+        after(s_out, s);
+        if (mode == kHostProject) {
+            if (plan->g.natoms > 0)
+                e = cudaMemcpy2DAsync(h_c, (size_t)nbands * row_bytes, d_c, (size_t)nb * row_bytes, (size_t)nb * row_bytes,
+                                      (size_t)plan->g.natoms, cudaMemcpyDeviceToHost, s_out);
+        } else {
+            e = cudaMemcpyAsync(h_psi, d_psi, band_bytes * nb, cudaMemcpyDeviceToHost, s_out);
+        }
+        if (e != cudaSuccess) return finish(cuda_fail(e, fn));
+        slot_free[slot] = mark(s_out);
+    }
+    after(s, s_out);
+    e = cudaStreamSynchronize(s);
+    for (cudaEvent_t ev : events) cudaEventDestroy(ev);
+    if (e != cudaSuccess) return cuda_fail(e, fn);
+    return SHO_OK;
+}
+
 sho_status sho_project_host(sho_plan* plan, const void* psi_host, int32_t nbands, void* coeff_host, void* cuda_stream)
 {
     sho_status st = check_hot("sho_project_host", plan, psi_host, coeff_host, nbands);
     if (st != SHO_OK) return st;
-    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-    const size_t esz = elem_size(plan->dtype);
-    const size_t band_bytes = (size_t)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * esz;
-    const size_t row_bytes = (size_t)plan->g.nsho * esz;                     // coefficients of one (atom, band)
-    const size_t c_bytes = (size_t)plan->g.natoms * nbands * row_bytes;
-    if ((st = ws_reserve(&plan->ws_psi, &plan->ws_psi_bytes, band_bytes * nbands, "sho_project_host")) != SHO_OK) return st;
-    if ((st = ws_reserve(&plan->ws_c, &plan->ws_c_bytes, std::max<size_t>(c_bytes, 16), "sho_project_host")) != SHO_OK) return st;
-    HostPipe hp;
-    if ((st = host_pipe_open(plan, s, &hp, "sho_project_host: streams")) != SHO_OK) return st;
-    const int cb = host_chunk_bands(plan, nbands);
-    cudaError_t e = cudaSuccess;
-    size_t c_off = 0;
-    for (int b0 = 0; b0 < nbands; b0 += cb) {
-        const int nb = std::min(cb, nbands - b0);
-        char* d_psi = static_cast<char*>(plan->ws_psi) + (size_t)b0 * band_bytes;
-        char* d_c = static_cast<char*>(plan->ws_c) + c_off;                   // [natoms][nb][N_SHO]
-        e = cudaMemcpyAsync(d_psi, static_cast<const char*>(psi_host) + (size_t)b0 * band_bytes, band_bytes * nb,
-                            cudaMemcpyHostToDevice, hp.s_in);
-        if (e != cudaSuccess) return cuda_fail(e, "sho_project_host: H2D psi");
-        hp.after(s, hp.s_in);
-        if (plan->g.natoms > 0) {
-            if ((st = launch_project(plan, d_psi, nb, d_c, s)) != SHO_OK) return st;
-            hp.after(hp.s_out, s);
-            e = cudaMemcpy2DAsync(static_cast<char*>(coeff_host) + (size_t)b0 * row_bytes, (size_t)nbands * row_bytes, d_c,
-                                  (size_t)nb * row_bytes, (size_t)nb * row_bytes, (size_t)plan->g.natoms,
-                                  cudaMemcpyDeviceToHost, hp.s_out);
-            if (e != cudaSuccess) return cuda_fail(e, "sho_project_host: D2H coeff");
-        }
-        c_off += (size_t)plan->g.natoms * nb * row_bytes;
-    }
-    hp.after(s, hp.s_out);
-    e = cudaStreamSynchronize(s);
-    if (e != cudaSuccess) return cuda_fail(e, "sho_project_host: synchronize");
-    return SHO_OK;
+    return host_run(plan, kHostProject, "sho_project_host", const_cast<void*>(psi_host), coeff_host, nullptr, nbands,
+                    static_cast<cudaStream_t>(cuda_stream));
 }
 
 sho_status sho_add_host(sho_plan* plan, const void* coeff_host, int32_t nbands, void* psi_host, void* cuda_stream)
 {
     sho_status st = check_hot("sho_add_host", plan, coeff_host, psi_host, nbands);
     if (st != SHO_OK) return st;
-    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-    const size_t esz = elem_size(plan->dtype);
-    const size_t band_bytes = (size_t)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * esz;
-    const size_t row_bytes = (size_t)plan->g.nsho * esz;
-    const size_t c_bytes = (size_t)plan->g.natoms * nbands * row_bytes;
     if (plan->g.natoms == 0 || plan->n_tile_list == 0) return SHO_OK;
-    if ((st = ws_reserve(&plan->ws_psi, &plan->ws_psi_bytes, band_bytes * nbands, "sho_add_host")) != SHO_OK) return st;
-    if ((st = ws_reserve(&plan->ws_c, &plan->ws_c_bytes, std::max<size_t>(c_bytes, 16), "sho_add_host")) != SHO_OK) return st;
-    HostPipe hp;
-    if ((st = host_pipe_open(plan, s, &hp, "sho_add_host: streams")) != SHO_OK) return st;
-    const int cb = host_chunk_bands(plan, nbands);
-    cudaError_t e = cudaSuccess;
-    size_t c_off = 0;
-    for (int b0 = 0; b0 < nbands; b0 += cb) {
-        const int nb = std::min(cb, nbands - b0);
-        char* d_psi = static_cast<char*>(plan->ws_psi) + (size_t)b0 * band_bytes;
-        char* d_c = static_cast<char*>(plan->ws_c) + c_off;                   // [natoms][nb][N_SHO]
-        e = cudaMemcpy2DAsync(d_c, (size_t)nb * row_bytes, static_cast<const char*>(coeff_host) + (size_t)b0 * row_bytes,
-                              (size_t)nbands * row_bytes, (size_t)nb * row_bytes, (size_t)plan->g.natoms,
-                              cudaMemcpyHostToDevice, hp.s_in);
-        if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: H2D coeff");
-        e = cudaMemcpyAsync(d_psi, static_cast<const char*>(psi_host) + (size_t)b0 * band_bytes, band_bytes * nb,
-                            cudaMemcpyHostToDevice, hp.s_in);
-        if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: H2D psi");
-        hp.after(s, hp.s_in);
-        if ((st = launch_add(plan, d_c, nb, d_psi, s)) != SHO_OK) return st;
-        hp.after(hp.s_out, s);
-        e = cudaMemcpyAsync(static_cast<char*>(psi_host) + (size_t)b0 * band_bytes, d_psi, band_bytes * nb,
-                            cudaMemcpyDeviceToHost, hp.s_out);
-        if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: D2H psi");
-        c_off += (size_t)plan->g.natoms * nb * row_bytes;
-    }
-    hp.after(s, hp.s_out);
-    e = cudaStreamSynchronize(s);
-    if (e != cudaSuccess) return cuda_fail(e, "sho_add_host: synchronize");
-    return SHO_OK;
+    return host_run(plan, kHostAdd, "sho_add_host", psi_host, const_cast<void*>(coeff_host), nullptr, nbands,
+                    static_cast<cudaStream_t>(cuda_stream));
+}
+
+sho_status sho_apply_host(sho_plan* plan, const double* dmat_host, void* psi_host, int32_t nbands, void* cuda_stream)
+{
+    sho_status st = check_hot("sho_apply_host", plan, dmat_host ? (const void*)dmat_host : psi_host, psi_host, nbands);
+    if (st != SHO_OK) return st;
+    if (plan->g.natoms == 0 || plan->n_tile_list == 0) return SHO_OK;
+    if (!dmat_host) { set_error("sho_apply_host: null argument"); return SHO_ERR_INVALID_ARG; }
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const size_t d_bytes = (size_t)plan->g.natoms * plan->g.nsho * plan->g.nsho * sizeof(double);
+    if ((st = ws_reserve(&plan->ws_d, &plan->ws_d_bytes, d_bytes, "sho_apply_host")) != SHO_OK) return st;
+    cudaError_t e = cudaMemcpyAsync(plan->ws_d, dmat_host, d_bytes, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(e, "sho_apply_host: H2D of the atomic matrices");
+    return host_run(plan, kHostApply, "sho_apply_host", psi_host, nullptr, static_cast<const double*>(plan->ws_d), nbands, s);
 }
 
 }  // extern "C"

@@ -100,6 +100,7 @@ struct sho_plan {
     // workspace for the *_host calls
     void* ws_psi; size_t ws_psi_bytes;
     void* ws_c;   size_t ws_c_bytes;
+    void* ws_d;   size_t ws_d_bytes;       // atomic matrices of sho_apply_host
     cudaStream_t s_in, s_out;              // copy streams of the *_host calls (created on first use)
 };
 
@@ -125,6 +126,7 @@ inline bool is_complex(sho_dtype t) { return t == SHO_C128 || t == SHO_C64; }
 // launchers (defined next to their kernels)
 sho_status launch_project(const sho_plan* p, const void* psi, int nbands, void* coeff, cudaStream_t s);
 sho_status launch_add(const sho_plan* p, const void* coeff, int nbands, void* psi, cudaStream_t s);
+sho_status launch_dmul(const sho_plan* p, const double* dmat, const void* cin, int nbands, void* cout, cudaStream_t s);
 sho_status launch_project_stored(const sho_plan* p, const sho_tables* t, const void* psi, int nbands, void* coeff,
                                  cudaStream_t s);
 sho_status tables_build(const sho_plan* p, sho_tables** out, size_t* bytes_needed, cudaStream_t s);

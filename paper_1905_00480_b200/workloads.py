@@ -95,6 +95,13 @@ class Workload:
             return out
         return rng.standard_normal(shape, dtype=real_t)
 
+    def dmatrix(self, nsho: int) -> np.ndarray:
+        """Synthetic atomic matrices D[natoms][nsho][nsho] of step (2) (eq. (28) PAPER.md:252-262:
+        real-valued, dimension N_SHO): fp64, symmetric, entries ~ N(0,1)/sqrt(nsho) (the real ones need PAW data)."""
+        rng = np.random.default_rng([self.seed, 11])
+        d = rng.standard_normal((self.natoms, int(nsho), int(nsho))) / np.sqrt(float(nsho))
+        return np.ascontiguousarray(0.5 * (d + np.transpose(d, (0, 2, 1))))
+
 
 def _lattice(rng, nsites, L, jitter):
     """Jittered simple-cubic sites (g + 1/2) L_d / n_d, z slowest, wrapped into the cell."""

@@ -510,6 +510,90 @@ def test_host_buffer_calls_pipeline_band_chunks(sho, k, chunk, monkeypatch):
         plan.close()
 
 
+# ------------------------------------------------------------------------------------------------
+# step (2) d = D c and the three-step non-local action
+
+
+@pytest.mark.parametrize("k,dtype", [(1, None), (2, None), (3, "r32"), (4, None), (5, None), (5, "c64")])
+def test_dmul_and_apply_match_the_oracle(sho, k, dtype):
+    """sho_dmul against oracle.dmul (not symmetric D: a transposed product fails), in place and out of place;
+    sho_apply against add(dmul(project(psi))) of the oracle; sho_apply_host (one upload of psi) against the same."""
+    import torch
+    w = workloads.make(k, size="small", dtype=dtype)
+    if dtype in ("r32", "r64"):
+        w.kfrac = None
+    tol = TOL[w.dtype]
+    wide = np.complex128 if w.is_complex else np.float64
+    plan = sho.plan_for(w)
+    try:
+        rng = np.random.default_rng(k)
+        D = rng.standard_normal((w.natoms, plan.nsho, plan.nsho)) / np.sqrt(plan.nsho)
+        c = w.coeff(plan.nsho)
+        ref = oracle.dmul(D, c.astype(wide))
+        d_D = _dev(D)
+        out = plan.dmul(d_D, _dev(c))
+        torch.cuda.synchronize()
+        scale = np.abs(ref).max()
+        assert np.abs(out.cpu().numpy().astype(wide) - ref).max() <= tol * scale
+        inpl = _dev(c)
+        plan.dmul(d_D, inpl, inpl)
+        torch.cuda.synchronize()
+        assert torch.equal(inpl, out), "in-place sho_dmul differs from out-of-place"
+        # the whole action with the workload's symmetric D
+        Dm = w.dmatrix(plan.nsho)
+        psi = w.psi()
+        if w.psi_dist == "zero":
+            psi = workloads.Workload(**{**w.__dict__, "psi_dist": "normal"}).psi()
+        geo = (w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax)
+        c_ref = oracle.project(*geo, psi.astype(wide), w.rcut_sigma)
+        psi_ref = oracle.add(*geo, oracle.dmul(Dm, c_ref), psi.astype(wide), w.rcut_sigma)
+        scale = np.maximum(np.abs(psi_ref).max(axis=(1, 2, 3)), 1e-300)
+        d_psi = _dev(psi)
+        work = plan.new_coeff(w.nbands)
+        plan.apply(_dev(Dm), d_psi, work)
+        torch.cuda.synchronize()
+        err = (np.abs(d_psi.cpu().numpy().astype(wide) - psi_ref).max(axis=(1, 2, 3)) / scale).max()
+        assert err <= tol, "sho_apply parity: %.3e > %.1e" % (err, tol)
+        d_ref = oracle.dmul(Dm, c_ref)
+        norm = _psi_norm(psi, w.h)
+        errd = (np.abs(work.cpu().numpy().astype(wide) - d_ref) / norm[None, :, None]).max()
+        assert errd <= tol * max(1.0, np.abs(Dm).sum(axis=2).max()), "coeff_work must hold d = D c on return"
+        host = psi.copy()
+        plan.apply_host(Dm, host)
+        err = (np.abs(host.astype(wide) - psi_ref).max(axis=(1, 2, 3)) / scale).max()
+        assert err <= tol, "sho_apply_host parity: %.3e > %.1e" % (err, tol)
+    finally:
+        plan.close()
+
+
+@pytest.mark.parametrize("chunk", ["1", "2"])
+def test_apply_host_pipelines_band_chunks_through_a_bounded_ring(sho, chunk, monkeypatch):
+    # 5 bands in chunks of 1 or 2: more chunks than the three ring slots, so slots are reused
+    monkeypatch.setenv("SHO_HOST_CHUNK_BANDS", chunk)
+    rng = np.random.default_rng(9)
+    ng = (24, 40, 16)
+    w = _custom(ng, (1, 1, 1), rng.uniform(0, 1, (6, 3)) * np.array(ng) * 0.25, rng.uniform(0.3, 0.36, 6), 5, 5, rc=4.0)
+    plan = sho.plan_for(w)
+    try:
+        Dm = w.dmatrix(plan.nsho)
+        psi = w.psi()
+        geo = (w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax)
+        c_ref = oracle.project(*geo, psi, w.rcut_sigma)
+        psi_ref = oracle.add(*geo, oracle.dmul(Dm, c_ref), psi, w.rcut_sigma)
+        host = psi.copy()
+        plan.apply_host(Dm, host)
+        assert np.abs(host - psi_ref).max() <= 1e-12 * np.abs(psi_ref).max()
+        c = np.zeros((w.natoms, w.nbands, plan.nsho))
+        plan.project_host(psi, c)
+        check_project(sho, w, psi, c, 1e-12)
+        out = psi.copy()
+        plan.add_host(c_ref, out)
+        ref = oracle.add(*geo, c_ref, psi, w.rcut_sigma)
+        assert np.abs(out - ref).max() <= 1e-12 * np.abs(ref).max()
+    finally:
+        plan.close()
+
+
 def test_wrong_arguments_raise(sho):
     import torch
     w = workloads.make(1)
