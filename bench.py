@@ -269,9 +269,17 @@ def run_ours(args, w):
     coeff = plan.new_coeff(nb, dev)
     stream = torch.cuda.current_stream()
 
+    bf = args.layout == "bf"
+    if bf:
+        psi = psi.permute(1, 2, 3, 0).contiguous()
+        psi_out = psi_out.permute(1, 2, 3, 0).contiguous()
+        work = torch.empty((min(nb, 64),) + shape[1:], dtype=tdt, device=dev)
+    do_project = (lambda: plan.project_bf(psi, coeff, work, stream)) if bf else (lambda: plan.project(psi, coeff, stream))
+    do_add = (lambda: plan.add_bf(coeff, psi_out, work, stream)) if bf else (lambda: plan.add(coeff, psi_out, stream))
+
     def step():
-        plan.project(psi, coeff, stream)
-        plan.add(coeff, psi_out, stream)
+        do_project()
+        do_add()
 
     def barrier():
         if world > 1:
@@ -286,9 +294,9 @@ def run_ours(args, w):
     barrier()
     for k in range(args.steps):
         ev[k][0].record(stream)
-        plan.project(psi, coeff, stream)
+        do_project()
         ev[k][1].record(stream)
-        plan.add(coeff, psi_out, stream)
+        do_add()
         ev[k][2].record(stream)
     barrier()
     clocks = sampler.stop() if sampler else None
@@ -312,6 +320,10 @@ def run_ours(args, w):
                 "flops_per_launch": F,
                 "frac_project": F / t_prj / 1e12 / alu_peak, "frac_add": F / t_add / 1e12 / alu_peak}
 
+    if bf:
+        args.no_e2e = args.no_stored = True      # the remaining legs use the native layout
+        psi_out = torch.zeros(shape, dtype=tdt, device=dev)
+        psi = psi.permute(3, 0, 1, 2).contiguous()
     # ---- the three-step action project -> D -> add in one call (f2), device resident, outside the timed region ----
     dmat = torch.from_numpy(w.dmatrix(plan.nsho)).to(dev)
     plan.apply(dmat, psi_out, coeff, stream)
@@ -399,7 +411,7 @@ def run_ours(args, w):
         "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": {"r64": "f64", "c128": "c128", "r32": "f32", "c64": "c64"}[w.dtype], "data": "synthetic",
         "config": {"workload": w.name, "grid": list(w.ng), "h": w.h, "natoms": w.natoms, "numax": w.numax, "nbands_per_gpu": nb,
-                   "elem": w.dtype, "l2": "inputs larger than L2 (psi %.2f GB per GPU)" % (np.prod(shape) * esz / 1e9)
+                   "elem": w.dtype, "layout": args.layout, "l2": "inputs larger than L2 (psi %.2f GB per GPU)" % (np.prod(shape) * esz / 1e9)
                    if np.prod(shape) * esz > 2.5e8 else "psi smaller than L2: L2-resident by design of the config",
                    "sharding": "bands (weak): each rank runs the config's nbands on its own psi, no collective"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps, "roofline": roofline, "cpu_baseline": cpu,
@@ -430,7 +442,11 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5 (default: the largest, cfg 5)")
+    ap.add_argument("--config", default="5", help="BASELINE.json config 1..5 (default: the largest, cfg 5), or 'paper': "
+                    "the paper's own benchmark (sec. 6: 64^3, fcc, 665 atoms, 1024 bands; --numax 0..5 = 1..56 coefficients)")
+    ap.add_argument("--numax", type=int, default=5, help="numax of --config paper")
+    ap.add_argument("--layout", default="xf", choices=["xf", "bf"], help="psi layout: x-fastest [b][z][y][x] (the ABI's native one) or "
+                    "band-fastest [z][y][x][b] (the paper's, PAPER.md:371; converted in chunks of 64 bands by sho_project_bf / sho_add_bf)")
     ap.add_argument("--dtype", default=None, help="override the config's element type (cfg 4: r32 or r64)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
@@ -438,7 +454,10 @@ def main():
     ap.add_argument("--no-stored", action="store_true", help="skip the stored-projector baseline leg")
     ap.add_argument("--ref-cpu-seconds", type=float, default=20.0)
     args = ap.parse_args()
-    w = workloads.make(args.config, dtype=args.dtype)
+    if args.config == "paper":
+        w = workloads.make_paper(args.numax, args.dtype or "r64")
+    else:
+        w = workloads.make(int(args.config), dtype=args.dtype)
     if args.dtype in ("r32", "r64"):
         w.kfrac = None
     if args.impl == "reference":

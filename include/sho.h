@@ -139,6 +139,20 @@ sho_status sho_apply(const sho_plan* plan, const double* dmat, void* psi, int32_
                      void* cuda_stream);
 
 /*
+ * Band-fastest psi layout psi_bf[Nz][Ny][Nx][nbands] -- the layout of the paper's own kernels, which vectorise
+ * over the band index.  The kernels of this library read x-fastest data, so these calls convert
+ * chunks of bands into the caller's workspace `work` (DEVICE, work_bytes >= the bytes of one band; an even number
+ * of bands per chunk is used when it fits) with a tiled transpose, run the same kernels on the chunk and, for
+ * the add-back, accumulate the chunk's increment into psi_bf with the inverse transpose.  coeff keeps the layout
+ * [natoms][nbands][N_SHO].  Asynchronous on the stream, allocates nothing.  SHO_ERR_INVALID_ARG if the workspace
+ * does not hold one band.
+ */
+sho_status sho_project_bf(const sho_plan* plan, const void* psi_bf, int32_t nbands, void* coeff, void* work, size_t work_bytes,
+                          void* cuda_stream);
+sho_status sho_add_bf(const sho_plan* plan, const void* coeff, int32_t nbands, void* psi_bf, void* work, size_t work_bytes,
+                      void* cuda_stream);
+
+/*
  * End-to-end variants with HOST buffers (pinned or pageable): copy in, run the same kernels, copy
  * out, and synchronise the stream before returning.  They use a device workspace owned by the plan
  * (the only hot-path calls that may allocate; it is grown on demand and bounded by the chunk size, not

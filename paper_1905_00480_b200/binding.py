@@ -85,6 +85,8 @@ def lib():
     L.sho_project_host.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
     L.sho_add_host.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
     L.sho_measure_fp64_peak.argtypes = [C.c_int32, _f64p]
+    L.sho_project_bf.argtypes = [_vp, _vp, C.c_int32, _vp, _vp, C.c_size_t, _vp]
+    L.sho_add_bf.argtypes = [_vp, _vp, C.c_int32, _vp, _vp, C.c_size_t, _vp]
     L.sho_dmul.argtypes = [_vp, _vp, _vp, C.c_int32, _vp, _vp]
     L.sho_apply.argtypes = [_vp, _vp, _vp, C.c_int32, _vp, _vp]
     L.sho_apply_host.argtypes = [_vp, _vp, _vp, C.c_int32, _vp]
@@ -277,6 +279,43 @@ class Plan:
                "sho_apply")
         return psi
 
+    # -- band-fastest psi [Nz][Ny][Nx][nbands] (the paper's layout) ------------------------------
+    def _check_psi_bf(self, psi, where):
+        torch = _torch()
+        if not (isinstance(psi, torch.Tensor) and psi.is_cuda and psi.is_contiguous() and psi.device.index == self.device):
+            raise ValueError("%s: psi_bf must be a contiguous CUDA tensor on the plan's device" % where)
+        if psi.dtype != _torch_dtype(self.dtype) or psi.dim() != 4 or tuple(psi.shape[:3]) != (self.ng[2], self.ng[1], self.ng[0]):
+            raise ValueError("%s: psi_bf must be [Nz][Ny][Nx][nbands] of the plan's dtype" % where)
+        return int(psi.shape[3])
+
+    def _work(self, work, nb, where):
+        torch = _torch()
+        if work is None:                 # convenience: a workspace of at most 64 bands
+            n = min(nb, 64)
+            work = torch.empty((n, self.ng[2], self.ng[1], self.ng[0]), dtype=_torch_dtype(self.dtype),
+                               device=torch.device("cuda", self.device))
+        if not (isinstance(work, torch.Tensor) and work.is_cuda and work.is_contiguous() and work.device.index == self.device):
+            raise ValueError("%s: work must be a contiguous CUDA tensor on the plan's device" % where)
+        return work
+
+    def project_bf(self, psi_bf, coeff=None, work=None, stream=None):
+        nb = self._check_psi_bf(psi_bf, "sho_project_bf")
+        if coeff is None:
+            coeff = self.new_coeff(nb, psi_bf.device)
+        self._check_coeff(coeff, nb, "sho_project_bf")
+        work = self._work(work, nb, "sho_project_bf")
+        _check(lib().sho_project_bf(self._h, psi_bf.data_ptr(), nb, coeff.data_ptr(), work.data_ptr(),
+                                    work.numel() * work.element_size(), _stream_handle(stream)), "sho_project_bf")
+        return coeff
+
+    def add_bf(self, coeff, psi_bf, work=None, stream=None):
+        nb = self._check_psi_bf(psi_bf, "sho_add_bf")
+        self._check_coeff(coeff, nb, "sho_add_bf")
+        work = self._work(work, nb, "sho_add_bf")
+        _check(lib().sho_add_bf(self._h, coeff.data_ptr(), nb, psi_bf.data_ptr(), work.data_ptr(),
+                                work.numel() * work.element_size(), _stream_handle(stream)), "sho_add_bf")
+        return psi_bf
+
     def tables_bytes(self) -> int:
         need = C.c_size_t(0)
         _check(lib().sho_tables_build(self._h, None, C.byref(need), None), "sho_tables_build(size query)")
@@ -352,6 +391,14 @@ def sho_add(plan: Plan, coeff, psi, stream=None):
 
 def sho_project_stored(plan: Plan, tables: Tables, psi, coeff=None, stream=None):
     return plan.project_stored(tables, psi, coeff, stream)
+
+
+def sho_project_bf(plan: Plan, psi_bf, coeff=None, work=None, stream=None):
+    return plan.project_bf(psi_bf, coeff, work, stream)
+
+
+def sho_add_bf(plan: Plan, coeff, psi_bf, work=None, stream=None):
+    return plan.add_bf(coeff, psi_bf, work, stream)
 
 
 def sho_dmul(plan: Plan, dmat, coeff, out=None, stream=None):

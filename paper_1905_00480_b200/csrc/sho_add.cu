@@ -50,6 +50,7 @@ struct AddParams {
     int32_t n_tile_list;
     int32_t nitems;            // work items = listed tiles x band chunks (one complex band or two real bands)
     int32_t nbands;
+    int32_t cnb;               // bands per atom in the coefficient array (>= nbands: a chunk of a wider array)
     int32_t ntile0, ntile1;
     int32_t vec_ok;
     int32_t rd;                // ring depth (pairs in flight between producers and XY warps)
@@ -488,7 +489,7 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
         double* fzw = FZ + (size_t)pw * FZS;
         real_t* stg = reinterpret_cast<real_t*>(STG + (size_t)pw * STGS);
         AddEntry* entw = ENTW + 2 * pw;
-        const size_t catom = (size_t)p.nbands * nsho * P;
+        const size_t catom = (size_t)p.cnb * nsho * P;
         // copy granule: one complex coefficient when its alignment is known, else one real number
         const int gran = (CPLX && p.vec_ok) ? 2 : 1;       // reals per cp.async
         // stream cursor: (citem, ci) is the work item that holds stream element cbase_s .. cbase_s + ci.z - 1;
@@ -634,7 +635,7 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
 }
 
 template <int KQ, int DT>
-static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s)
+static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb)
 {
     using S = AddSmem<KQ>;
     constexpr bool CPLX = Elem<DT>::cplx;
@@ -647,6 +648,7 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
     p.cidx = pl->d_cidx; p.t2pos = pl->d_t2pos;
     p.n_tile_list = pl->n_tile_list;
     p.nbands = nbands;
+    p.cnb = cnb;
     p.ntile0 = pl->ntile[0]; p.ntile1 = pl->ntile[1];
     p.band_stride = (long long)pl->g.ng[0] * pl->g.ng[1] * pl->g.ng[2];
     const size_t esz = elem_size(pl->dtype);
@@ -689,23 +691,24 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
 }
 
 template <int DT>
-static sho_status launch_kq(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s)
+static sho_status launch_kq(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb)
 {
     switch ((pl->g.numax + 4) >> 2) {          // K steps of four n values that hold n <= numax
-        case 1: return launch_t<1, DT>(pl, coeff, nbands, psi, s);
-        case 2: return launch_t<2, DT>(pl, coeff, nbands, psi, s);
-        case 3: return launch_t<3, DT>(pl, coeff, nbands, psi, s);
-        default: return launch_t<4, DT>(pl, coeff, nbands, psi, s);
+        case 1: return launch_t<1, DT>(pl, coeff, nbands, psi, s, cnb);
+        case 2: return launch_t<2, DT>(pl, coeff, nbands, psi, s, cnb);
+        case 3: return launch_t<3, DT>(pl, coeff, nbands, psi, s, cnb);
+        default: return launch_t<4, DT>(pl, coeff, nbands, psi, s, cnb);
     }
 }
 
-sho_status launch_add(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s)
+sho_status launch_add(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb)
 {
+    if (cnb <= 0) cnb = nbands;
     switch (pl->dtype) {
-        case SHO_R64:  return launch_kq<SHO_R64>(pl, coeff, nbands, psi, s);
-        case SHO_C128: return launch_kq<SHO_C128>(pl, coeff, nbands, psi, s);
-        case SHO_R32:  return launch_kq<SHO_R32>(pl, coeff, nbands, psi, s);
-        case SHO_C64:  return launch_kq<SHO_C64>(pl, coeff, nbands, psi, s);
+        case SHO_R64:  return launch_kq<SHO_R64>(pl, coeff, nbands, psi, s, cnb);
+        case SHO_C128: return launch_kq<SHO_C128>(pl, coeff, nbands, psi, s, cnb);
+        case SHO_R32:  return launch_kq<SHO_R32>(pl, coeff, nbands, psi, s, cnb);
+        case SHO_C64:  return launch_kq<SHO_C64>(pl, coeff, nbands, psi, s, cnb);
     }
     set_error("sho_add: bad dtype");
     return SHO_ERR_INVALID_ARG;

@@ -507,6 +507,63 @@ sho_status sho_apply(const sho_plan* plan, const double* dmat, void* psi, int32_
     return launch_add(plan, coeff_work, nbands, psi, s);
 }
 
+// ---- band-fastest psi layout (the paper's own layout) ---------------------------------
+static sho_status bf_chunk(const char* fn, const sho_plan* plan, int32_t nbands, size_t work_bytes, int* cb)
+{
+    const size_t band_bytes = (size_t)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * elem_size(plan->dtype);
+    size_t n = band_bytes ? work_bytes / band_bytes : (size_t)nbands;
+    if (n > 1) n -= n & 1;                       // an even number of bands: the add kernel pairs real bands
+    if (n < 1) {
+        set_error("%s: the workspace of %zu bytes does not hold one band (%zu bytes)", fn, work_bytes, band_bytes);
+        return SHO_ERR_INVALID_ARG;
+    }
+    *cb = (int)std::min<size_t>(n, (size_t)nbands);
+    return SHO_OK;
+}
+
+sho_status sho_project_bf(const sho_plan* plan, const void* psi_bf, int32_t nbands, void* coeff, void* work, size_t work_bytes,
+                          void* cuda_stream)
+{
+    if (plan && plan->g.natoms == 0 && psi_bf && nbands > 0) return SHO_OK;
+    sho_status st = check_hot("sho_project_bf", plan, psi_bf, coeff, nbands);
+    if (st != SHO_OK) return st;
+    if (!work) { set_error("sho_project_bf: null workspace"); return SHO_ERR_INVALID_ARG; }
+    int cb = 0;
+    if ((st = bf_chunk("sho_project_bf", plan, nbands, work_bytes, &cb)) != SHO_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const size_t row = (size_t)plan->g.nsho * elem_size(plan->dtype);
+    for (int b0 = 0; b0 < nbands; b0 += cb) {
+        const int nb = std::min(cb, nbands - b0);
+        if ((st = launch_to_x_fastest(plan, psi_bf, nbands, b0, nb, work, s)) != SHO_OK) return st;
+        if ((st = launch_project(plan, work, nb, static_cast<char*>(coeff) + (size_t)b0 * row, s, nbands)) != SHO_OK) return st;
+    }
+    return SHO_OK;
+}
+
+sho_status sho_add_bf(const sho_plan* plan, const void* coeff, int32_t nbands, void* psi_bf, void* work, size_t work_bytes,
+                      void* cuda_stream)
+{
+    if (plan && plan->g.natoms == 0 && psi_bf && nbands > 0) return SHO_OK;
+    sho_status st = check_hot("sho_add_bf", plan, coeff, psi_bf, nbands);
+    if (st != SHO_OK) return st;
+    if (!work) { set_error("sho_add_bf: null workspace"); return SHO_ERR_INVALID_ARG; }
+    if (plan->n_tile_list == 0) return SHO_OK;
+    int cb = 0;
+    if ((st = bf_chunk("sho_add_bf", plan, nbands, work_bytes, &cb)) != SHO_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const size_t band_bytes = (size_t)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * elem_size(plan->dtype);
+    const size_t row = (size_t)plan->g.nsho * elem_size(plan->dtype);
+    for (int b0 = 0; b0 < nbands; b0 += cb) {
+        const int nb = std::min(cb, nbands - b0);
+        // the chunk's increment A c is built in the (zeroed) workspace, then accumulated into psi_bf in one pass
+        cudaError_t e = cudaMemsetAsync(work, 0, band_bytes * nb, s);
+        if (e != cudaSuccess) return cuda_fail(e, "sho_add_bf: memset");
+        if ((st = launch_add(plan, static_cast<const char*>(coeff) + (size_t)b0 * row, nb, work, s, nbands)) != SHO_OK) return st;
+        if ((st = launch_from_x_fastest(plan, work, nbands, b0, nb, psi_bf, s)) != SHO_OK) return st;
+    }
+    return SHO_OK;
+}
+
 // ---- HOST-buffer end-to-end variants ------------------------------------------------------------
 static sho_status ws_reserve(void** ws, size_t* have, size_t need, const char* what)
 {

@@ -124,8 +124,11 @@ inline size_t elem_size(sho_dtype t) { return t == SHO_R64 ? 8 : t == SHO_C128 ?
 inline bool is_complex(sho_dtype t) { return t == SHO_C128 || t == SHO_C64; }
 
 // launchers (defined next to their kernels)
-sho_status launch_project(const sho_plan* p, const void* psi, int nbands, void* coeff, cudaStream_t s);
-sho_status launch_add(const sho_plan* p, const void* coeff, int nbands, void* psi, cudaStream_t s);
+// cnb: bands per atom in the coefficient array when the launch covers a chunk of a wider array (0: nbands)
+sho_status launch_project(const sho_plan* p, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb = 0);
+sho_status launch_add(const sho_plan* p, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb = 0);
+sho_status launch_to_x_fastest(const sho_plan* p, const void* psi_bf, int nbands, int b0, int nb, void* psi_xf, cudaStream_t s);
+sho_status launch_from_x_fastest(const sho_plan* p, const void* psi_xf, int nbands, int b0, int nb, void* psi_bf, cudaStream_t s);
 sho_status launch_dmul(const sho_plan* p, const double* dmat, const void* cin, int nbands, void* cout, cudaStream_t s);
 sho_status launch_project_stored(const sho_plan* p, const sho_tables* t, const void* psi, int nbands, void* coeff,
                                  cudaStream_t s);

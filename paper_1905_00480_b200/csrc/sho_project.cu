@@ -42,6 +42,7 @@ struct ProjParams {
     const int32_t* order;
     const uint32_t* nxyz;
     int32_t nbands;
+    int32_t cnb;               // bands per atom in the coefficient array (>= nbands: a chunk of a wider array)
     int32_t n_work_atoms;      // atoms with a non-empty box (first entries of order[])
     int32_t kx_cap, yb_cap, nz_cap;    // capacities of the shared tables: x steps, 8-row blocks, planes
     int32_t fast;              // 32-byte loads are legal: psi 32-byte aligned and Nx a multiple of the lane span
@@ -552,7 +553,7 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
 
     // ---- store: c[a][b][n] = h^3 * acc (reading A7) ----
     const double h3 = p.g.h * p.g.h * p.g.h;
-    real_t* cout = reinterpret_cast<real_t*>(p.coeff) + ((size_t)a * p.nbands + b) * p.g.nsho * P;
+    real_t* cout = reinterpret_cast<real_t*>(p.coeff) + ((size_t)a * p.cnb + b) * p.g.nsho * P;
 #pragma unroll
     for (int j = 0; j < NACC; ++j) {
         const int n = tid + j * blockDim.x;
@@ -564,17 +565,17 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
 }
 
 template <typename T>
-__global__ void sho_zero_empty_kernel(T* coeff, const int32_t* order, int first, int count, int nbands, int nvals)
+__global__ void sho_zero_empty_kernel(T* coeff, const int32_t* order, int first, int count, int nbands, int nvals, int cnb)
 {
     // atoms with an empty box (isolated grid, atom outside): coefficients are exact zeros
     const int a = order[first + blockIdx.x];
-    T* c = coeff + (size_t)a * nbands * nvals;
+    T* c = coeff + (size_t)a * cnb * nvals;
     for (int i = threadIdx.x; i < nbands * nvals; i += blockDim.x) c[i] = (T)0;
     (void)count;
 }
 
 template <int MT, int R, int DT, int G>
-static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s)
+static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb)
 {
     using S = ProjSmem<MT, R, DT>;
     constexpr bool CPLX = Elem<DT>::cplx;
@@ -584,6 +585,7 @@ static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void
     p.psi = psi; p.coeff = coeff;
     p.atoms = pl->d_atoms; p.order = pl->d_order; p.nxyz = pl->d_nxyz;
     p.nbands = nbands;
+    p.cnb = cnb;
     p.n_work_atoms = pl->n_nonempty;
     p.kx_cap = (pl->max_n[0] + 2 * (CWX - 1)) / CWX + 2;     // + the twice-scheduled image-boundary step
     p.yb_cap = (pl->max_n[1] + 7) / 8 + 1;
@@ -611,7 +613,7 @@ static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void
         using real_t = typename Elem<DT>::real_t;
         sho_zero_empty_kernel<real_t><<<nempty, 256, 0, s>>>(reinterpret_cast<real_t*>(coeff), pl->d_order,
                                                               pl->n_nonempty, nempty, nbands,
-                                                              pl->g.nsho * (CPLX ? 2 : 1));
+                                                              pl->g.nsho * (CPLX ? 2 : 1), cnb);
         e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(e, "launch sho_zero_empty_kernel");
     }
@@ -619,32 +621,33 @@ static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void
 }
 
 template <int DT, int G>
-static sho_status launch_mg(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s)
+static sho_status launch_mg(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb)
 {
     // numax + 1 functions per axis: <= 8 one MMA row tile; 9, 10 one tile + 2 DFMA rows; more: two tiles
     const int M = pl->g.numax + 1;
-    if (M <= 8) return launch_t<1, 0, DT, G>(pl, psi, nbands, coeff, s);
-    if (M <= 10) return launch_t<1, 2, DT, G>(pl, psi, nbands, coeff, s);
-    return launch_t<2, 0, DT, G>(pl, psi, nbands, coeff, s);
+    if (M <= 8) return launch_t<1, 0, DT, G>(pl, psi, nbands, coeff, s, cnb);
+    if (M <= 10) return launch_t<1, 2, DT, G>(pl, psi, nbands, coeff, s, cnb);
+    return launch_t<2, 0, DT, G>(pl, psi, nbands, coeff, s, cnb);
 }
 
 template <int DT>
-static sho_status launch_m(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s)
+static sho_status launch_m(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb)
 {
     // Loads are issued kProjG = 2 steps at a time (longer prefetch distance); a row block with an odd number of
     // steps then wastes one.  Real data has few, long steps (16 or 32 columns): when more than 6 % of them would
     // be lost, issue them one by one (cfg 3: 4-5 steps per row block, 1.90 vs 2.03 ms; cfg 4: 8, 15.5 vs 16.1 ms).
-    if (!Elem<DT>::cplx && pl->proj_odd_steps > 0.06) return launch_mg<DT, 1>(pl, psi, nbands, coeff, s);
-    return launch_mg<DT, kProjG>(pl, psi, nbands, coeff, s);
+    if (!Elem<DT>::cplx && pl->proj_odd_steps > 0.06) return launch_mg<DT, 1>(pl, psi, nbands, coeff, s, cnb);
+    return launch_mg<DT, kProjG>(pl, psi, nbands, coeff, s, cnb);
 }
 
-sho_status launch_project(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s)
+sho_status launch_project(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb)
 {
+    if (cnb <= 0) cnb = nbands;
     switch (pl->dtype) {
-        case SHO_R64:  return launch_m<SHO_R64>(pl, psi, nbands, coeff, s);
-        case SHO_C128: return launch_m<SHO_C128>(pl, psi, nbands, coeff, s);
-        case SHO_R32:  return launch_m<SHO_R32>(pl, psi, nbands, coeff, s);
-        case SHO_C64:  return launch_m<SHO_C64>(pl, psi, nbands, coeff, s);
+        case SHO_R64:  return launch_m<SHO_R64>(pl, psi, nbands, coeff, s, cnb);
+        case SHO_C128: return launch_m<SHO_C128>(pl, psi, nbands, coeff, s, cnb);
+        case SHO_R32:  return launch_m<SHO_R32>(pl, psi, nbands, coeff, s, cnb);
+        case SHO_C64:  return launch_m<SHO_C64>(pl, psi, nbands, coeff, s, cnb);
     }
     set_error("sho_project: bad dtype");
     return SHO_ERR_INVALID_ARG;

@@ -594,6 +594,47 @@ def test_apply_host_pipelines_band_chunks_through_a_bounded_ring(sho, chunk, mon
         plan.close()
 
 
+# ------------------------------------------------------------------------------------------------
+# the paper's own workload (sec. 6) and its band-fastest psi layout
+
+
+@pytest.mark.parametrize("numax,dtype", [(0, "r64"), (2, "r64"), (5, "r64"), (4, "r32")])
+def test_paper_workload_small(sho, numax, dtype):
+    """PAPER.md:369-377 at 24^3 points / 16 bands: isolated domain, fcc atoms of which most sit outside the grid
+    with a clipped region; full comparison with the oracle."""
+    run_case(sho, workloads.make_paper(numax, dtype, size="small"))
+
+
+@pytest.mark.parametrize("dtype,nb,wb", [("r64", 16, 16), ("r64", 7, 2), ("r32", 5, 1), ("c128", 3, 2)])
+def test_band_fastest_layout_entry_points(sho, dtype, nb, wb):
+    """sho_project_bf / sho_add_bf on psi_bf[Nz][Ny][Nx][nbands] against the oracle on the transposed
+    data, with workspaces of wb bands (several chunks, ragged last chunk, odd band counts)."""
+    import torch
+    w = workloads.make_paper(3, dtype, size="small") if dtype != "c128" else workloads.make(5, size="small")
+    w.nbands = nb
+    tol = TOL[w.dtype]
+    wide = np.complex128 if w.is_complex else np.float64
+    plan = sho.plan_for(w)
+    try:
+        psi = w.psi()                                              # [nb][Nz][Ny][Nx]
+        psi_bf = _dev(np.ascontiguousarray(np.moveaxis(psi, 0, 3)))
+        work = torch.empty((wb, w.ng[2], w.ng[1], w.ng[0]), dtype=psi_bf.dtype, device="cuda")
+        c = plan.project_bf(psi_bf, work=work)
+        torch.cuda.synchronize()
+        check_project(sho, w, psi, c.cpu().numpy(), tol)
+        coeff = w.coeff(plan.nsho)
+        plan.add_bf(_dev(coeff), psi_bf, work=work)
+        torch.cuda.synchronize()
+        ref = oracle.add(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax, coeff.astype(wide), psi.astype(wide), w.rcut_sigma)
+        got = np.moveaxis(psi_bf.cpu().numpy(), 3, 0).astype(wide)
+        scale = np.abs(ref).max(axis=(1, 2, 3))
+        assert (np.abs(got - ref).max(axis=(1, 2, 3)) / scale).max() <= tol
+        with pytest.raises(sho.ShoError):
+            plan.project_bf(psi_bf, work=torch.empty(8, dtype=psi_bf.dtype, device="cuda"))
+    finally:
+        plan.close()
+
+
 def test_wrong_arguments_raise(sho):
     import torch
     w = workloads.make(1)
