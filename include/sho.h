@@ -64,6 +64,7 @@ typedef enum { SHO_R64 = 0, SHO_C128 = 1, SHO_R32 = 2, SHO_C64 = 3 } sho_dtype;
 
 typedef struct sho_plan sho_plan;     /* opaque, library-owned: geometry of one set of atoms on one grid */
 typedef struct sho_tables sho_tables; /* opaque, library-owned: pre-sampled 3D projector tables          */
+typedef struct sho_tables1d sho_tables1d; /* opaque, library-owned: pre-sampled 1D factor tables          */
 
 /* eq. (18): (numax+1)(numax+2)(numax+3)/6; -1 if numax is outside [0, SHO_NUMAX_MAX] */
 int sho_nsho(int numax);
@@ -137,6 +138,28 @@ sho_status sho_dmul(const sho_plan* plan, const double* dmat, const void* coeff_
  */
 sho_status sho_apply(const sho_plan* plan, const double* dmat, void* psi, int32_t nbands, void* coeff_work,
                      void* cuda_stream);
+
+/*
+ * The stored add-back, the paper's "USUadd" (tab. 1): psi += A coeff reading the same
+ * pre-sampled 3D tables as sho_project_stored.  A baseline: its results meet in psi by atomicAdd, so it
+ * is correct to rounding but not bit-reproducible.
+ */
+sho_status sho_add_stored(const sho_plan* plan, const sho_tables* tables, const void* coeff, int32_t nbands, void* psi,
+                          void* cuda_stream);
+
+/*
+ * Stored-1D-table separable variant (sec. 3.4, eq. (22)-(23)): the same separable kernels
+ * as sho_project / sho_add, but the 1D factor values phi_n(u) of every atom and box index are read from
+ * device memory (pre-sampled by sho_tables1d_build: (n_x + n_y + n_z)(numax + 1) doubles per atom) instead
+ * of being generated by the recurrence.  Separates the gain of factorisation from the gain of on-the-fly
+ * sampling.  *bytes_needed is always filled; out = NULL queries the size only.
+ */
+sho_status sho_tables1d_build(const sho_plan* plan, sho_tables1d** out, size_t* bytes_needed, void* cuda_stream);
+sho_status sho_tables1d_destroy(sho_tables1d* tables);
+sho_status sho_project_stored1d(const sho_plan* plan, const sho_tables1d* tables, const void* psi, int32_t nbands,
+                                void* coeff, void* cuda_stream);
+sho_status sho_add_stored1d(const sho_plan* plan, const sho_tables1d* tables, const void* coeff, int32_t nbands,
+                            void* psi, void* cuda_stream);
 
 /*
  * Band-fastest psi layout psi_bf[Nz][Ny][Nx][nbands] -- the layout of the paper's own kernels, which vectorise

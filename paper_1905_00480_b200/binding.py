@@ -85,6 +85,11 @@ def lib():
     L.sho_project_host.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
     L.sho_add_host.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
     L.sho_measure_fp64_peak.argtypes = [C.c_int32, _f64p]
+    L.sho_add_stored.argtypes = [_vp, _vp, _vp, C.c_int32, _vp, _vp]
+    L.sho_tables1d_build.argtypes = [_vp, C.POINTER(_vp), C.POINTER(C.c_size_t), _vp]
+    L.sho_tables1d_destroy.argtypes = [_vp]
+    L.sho_project_stored1d.argtypes = [_vp, _vp, _vp, C.c_int32, _vp, _vp]
+    L.sho_add_stored1d.argtypes = [_vp, _vp, _vp, C.c_int32, _vp, _vp]
     L.sho_project_bf.argtypes = [_vp, _vp, C.c_int32, _vp, _vp, C.c_size_t, _vp]
     L.sho_add_bf.argtypes = [_vp, _vp, C.c_int32, _vp, _vp, C.c_size_t, _vp]
     L.sho_dmul.argtypes = [_vp, _vp, _vp, C.c_int32, _vp, _vp]
@@ -143,6 +148,15 @@ class Tables:
             self.close()
         except Exception:
             pass
+
+
+class Tables1D(Tables):
+    """Pre-sampled 1D factor tables (the stored-1D separable variant); owned by the library."""
+
+    def close(self):
+        if self._h:
+            lib().sho_tables1d_destroy(self._h)
+            self._h = None
 
 
 class Plan:
@@ -337,6 +351,39 @@ class Plan:
                                         _stream_handle(stream)), "sho_project_stored")
         return coeff
 
+    def add_stored(self, tables, coeff, psi, stream=None):
+        nb = self._check_psi(psi, "sho_add_stored")
+        self._check_coeff(coeff, nb, "sho_add_stored")
+        _check(lib().sho_add_stored(self._h, tables._h, coeff.data_ptr(), nb, psi.data_ptr(), _stream_handle(stream)), "sho_add_stored")
+        return psi
+
+    def tables1d_bytes(self) -> int:
+        need = C.c_size_t(0)
+        _check(lib().sho_tables1d_build(self._h, None, C.byref(need), None), "sho_tables1d_build(size query)")
+        return int(need.value)
+
+    def tables1d(self, stream=None) -> Tables1D:
+        need = C.c_size_t(0)
+        h_ = _vp()
+        _check(lib().sho_tables1d_build(self._h, C.byref(h_), C.byref(need), _stream_handle(stream)), "sho_tables1d_build")
+        return Tables1D(self, h_, need.value)
+
+    def project_stored1d(self, tables, psi, coeff=None, stream=None):
+        nb = self._check_psi(psi, "sho_project_stored1d")
+        if coeff is None:
+            coeff = self.new_coeff(nb, psi.device)
+        self._check_coeff(coeff, nb, "sho_project_stored1d")
+        _check(lib().sho_project_stored1d(self._h, tables._h, psi.data_ptr(), nb, coeff.data_ptr(), _stream_handle(stream)),
+               "sho_project_stored1d")
+        return coeff
+
+    def add_stored1d(self, tables, coeff, psi, stream=None):
+        nb = self._check_psi(psi, "sho_add_stored1d")
+        self._check_coeff(coeff, nb, "sho_add_stored1d")
+        _check(lib().sho_add_stored1d(self._h, tables._h, coeff.data_ptr(), nb, psi.data_ptr(), _stream_handle(stream)),
+               "sho_add_stored1d")
+        return psi
+
     # -- end-to-end with HOST buffers (numpy arrays or pinned CPU tensors) ------------------------
     def _host_ptr(self, a, shape, where):
         torch = _torch()
@@ -391,6 +438,18 @@ def sho_add(plan: Plan, coeff, psi, stream=None):
 
 def sho_project_stored(plan: Plan, tables: Tables, psi, coeff=None, stream=None):
     return plan.project_stored(tables, psi, coeff, stream)
+
+
+def sho_add_stored(plan: Plan, tables: Tables, coeff, psi, stream=None):
+    return plan.add_stored(tables, coeff, psi, stream)
+
+
+def sho_project_stored1d(plan: Plan, tables: Tables1D, psi, coeff=None, stream=None):
+    return plan.project_stored1d(tables, psi, coeff, stream)
+
+
+def sho_add_stored1d(plan: Plan, tables: Tables1D, coeff, psi, stream=None):
+    return plan.add_stored1d(tables, coeff, psi, stream)
 
 
 def sho_project_bf(plan: Plan, psi_bf, coeff=None, work=None, stream=None):

@@ -45,6 +45,8 @@ struct AddParams {
     void* psi;
     const int4* tile_info;     // per listed tile: (tile, first entry, entries, 0)
     const AddEntry* tile_ent;
+    const double* tab1d;       // stored 1D tables (sho_add_stored1d), or null: sample on the fly
+    const long long* tab1d_off;
     const uint16_t* cidx;      // [nblk][32] coefficient index held by lane 4 q + t of z-stage K block (0xffff: none)
     const uint16_t* t2pos;
     int32_t n_tile_list;
@@ -566,7 +568,9 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
                     const int iu = j + (int)en->m[d] * N;
                     const bool valid = j < N && iu >= en->lo[d] && iu <= en->hi[d];
                     double v[NV];
-                    if (valid) {
+                    if (valid && p.tab1d) {
+                        stored1d_lookup<NV>(p.tab1d, p.tab1d_off[en->atom], en->lo, en->hi, d, iu, p.g.numax, true, v);
+                    } else if (valid) {
                         hermite_gauss_s<NV>(displacement(iu, p.g.h, en->pos[d]), inv_sigma, pref, p.hz, EXPT, v);
                     } else {
 #pragma unroll
@@ -635,7 +639,7 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
 }
 
 template <int KQ, int DT>
-static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb)
+static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb, const sho_tables1d* t1)
 {
     using S = AddSmem<KQ>;
     constexpr bool CPLX = Elem<DT>::cplx;
@@ -645,6 +649,7 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
     p.zt = pl->ztiles;
     p.coeff = coeff; p.psi = psi;
     p.tile_info = pl->d_tile_info; p.tile_ent = pl->d_tile_ent;
+    p.tab1d = t1 ? t1->d_data : nullptr; p.tab1d_off = t1 ? t1->d_atom_off : nullptr;
     p.cidx = pl->d_cidx; p.t2pos = pl->d_t2pos;
     p.n_tile_list = pl->n_tile_list;
     p.nbands = nbands;
@@ -691,24 +696,24 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
 }
 
 template <int DT>
-static sho_status launch_kq(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb)
+static sho_status launch_kq(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb, const sho_tables1d* t1)
 {
     switch ((pl->g.numax + 4) >> 2) {          // K steps of four n values that hold n <= numax
-        case 1: return launch_t<1, DT>(pl, coeff, nbands, psi, s, cnb);
-        case 2: return launch_t<2, DT>(pl, coeff, nbands, psi, s, cnb);
-        case 3: return launch_t<3, DT>(pl, coeff, nbands, psi, s, cnb);
-        default: return launch_t<4, DT>(pl, coeff, nbands, psi, s, cnb);
+        case 1: return launch_t<1, DT>(pl, coeff, nbands, psi, s, cnb, t1);
+        case 2: return launch_t<2, DT>(pl, coeff, nbands, psi, s, cnb, t1);
+        case 3: return launch_t<3, DT>(pl, coeff, nbands, psi, s, cnb, t1);
+        default: return launch_t<4, DT>(pl, coeff, nbands, psi, s, cnb, t1);
     }
 }
 
-sho_status launch_add(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb)
+sho_status launch_add(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb, const sho_tables1d* t1)
 {
     if (cnb <= 0) cnb = nbands;
     switch (pl->dtype) {
-        case SHO_R64:  return launch_kq<SHO_R64>(pl, coeff, nbands, psi, s, cnb);
-        case SHO_C128: return launch_kq<SHO_C128>(pl, coeff, nbands, psi, s, cnb);
-        case SHO_R32:  return launch_kq<SHO_R32>(pl, coeff, nbands, psi, s, cnb);
-        case SHO_C64:  return launch_kq<SHO_C64>(pl, coeff, nbands, psi, s, cnb);
+        case SHO_R64:  return launch_kq<SHO_R64>(pl, coeff, nbands, psi, s, cnb, t1);
+        case SHO_C128: return launch_kq<SHO_C128>(pl, coeff, nbands, psi, s, cnb, t1);
+        case SHO_R32:  return launch_kq<SHO_R32>(pl, coeff, nbands, psi, s, cnb, t1);
+        case SHO_C64:  return launch_kq<SHO_C64>(pl, coeff, nbands, psi, s, cnb, t1);
     }
     set_error("sho_add: bad dtype");
     return SHO_ERR_INVALID_ARG;

@@ -469,6 +469,7 @@ sho_status sho_tables_destroy(sho_tables* t)
     cudaFree(t->d_atom_off);
     cudaFree(t->d_seg_atom);
     cudaFree(t->d_seg_qz0);
+    cudaFree(t->d_turn);
     delete t;
     return SHO_OK;
 }
@@ -505,6 +506,58 @@ sho_status sho_apply(const sho_plan* plan, const double* dmat, void* psi, int32_
     if ((st = launch_dmul(plan, dmat, coeff_work, nbands, coeff_work, s)) != SHO_OK) return st;
     if (plan->n_tile_list == 0) return SHO_OK;
     return launch_add(plan, coeff_work, nbands, psi, s);
+}
+
+// ---- stored variants beyond the 3D projection (f3) ---------------------------------------------------
+sho_status sho_add_stored(const sho_plan* plan, const sho_tables* tables, const void* coeff, int32_t nbands, void* psi,
+                          void* cuda_stream)
+{
+    if (plan && plan->g.natoms == 0 && psi && nbands > 0 && tables && tables->plan == plan && tables->plan_serial == plan->serial) return SHO_OK;
+    sho_status st = check_hot("sho_add_stored", plan, coeff, psi, nbands);
+    if (st != SHO_OK) return st;
+    if (!tables || tables->plan != plan || tables->plan_serial != plan->serial) { set_error("sho_add_stored: tables do not belong to this plan"); return SHO_ERR_INVALID_ARG; }
+    return launch_add_stored(plan, tables, coeff, nbands, psi, static_cast<cudaStream_t>(cuda_stream));
+}
+
+sho_status sho_tables1d_build(const sho_plan* plan, sho_tables1d** out, size_t* bytes_needed, void* cuda_stream)
+{
+    if (out) *out = nullptr;
+    if (!plan || !bytes_needed) { set_error("sho_tables1d_build: null argument"); return SHO_ERR_INVALID_ARG; }
+    return tables1d_build(plan, out, bytes_needed, static_cast<cudaStream_t>(cuda_stream));
+}
+
+sho_status sho_tables1d_destroy(sho_tables1d* t)
+{
+    if (!t) return SHO_OK;
+    cudaFree(t->d_data);
+    cudaFree(t->d_atom_off);
+    delete t;
+    return SHO_OK;
+}
+
+static sho_status check_t1(const char* fn, const sho_plan* plan, const sho_tables1d* t)
+{
+    if (!t || t->plan != plan || t->plan_serial != plan->serial) { set_error("%s: tables do not belong to this plan", fn); return SHO_ERR_INVALID_ARG; }
+    return SHO_OK;
+}
+
+sho_status sho_project_stored1d(const sho_plan* plan, const sho_tables1d* tables, const void* psi, int32_t nbands, void* coeff,
+                                void* cuda_stream)
+{
+    if (plan && plan->g.natoms == 0 && psi && nbands > 0) return SHO_OK;
+    sho_status st = check_hot("sho_project_stored1d", plan, psi, coeff, nbands);
+    if (st != SHO_OK || (st = check_t1("sho_project_stored1d", plan, tables)) != SHO_OK) return st;
+    return launch_project(plan, psi, nbands, coeff, static_cast<cudaStream_t>(cuda_stream), 0, tables);
+}
+
+sho_status sho_add_stored1d(const sho_plan* plan, const sho_tables1d* tables, const void* coeff, int32_t nbands, void* psi,
+                            void* cuda_stream)
+{
+    if (plan && plan->g.natoms == 0 && psi && nbands > 0) return SHO_OK;
+    sho_status st = check_hot("sho_add_stored1d", plan, coeff, psi, nbands);
+    if (st != SHO_OK || (st = check_t1("sho_add_stored1d", plan, tables)) != SHO_OK) return st;
+    if (plan->n_tile_list == 0) return SHO_OK;
+    return launch_add(plan, coeff, nbands, psi, static_cast<cudaStream_t>(cuda_stream), 0, tables);
 }
 
 // ---- band-fastest psi layout (the paper's own layout) ---------------------------------

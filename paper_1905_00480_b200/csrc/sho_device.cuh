@@ -89,6 +89,23 @@ __device__ __forceinline__ void hermite_gauss(double u, const AtomDev& at, const
     }
 }
 
+// The stored-1D-table variant (f3: the factor matrices v[x], v[y], v[z] of eq. (22)-(23) read from
+// memory instead of being generated): per atom the rows phi_0..phi_numax of every box index of the x, then y, then z
+// axis, M = numax + 1 doubles per index.  Returns the M values of axis d at unwrapped index i (zeros beyond numax or
+// when !valid).
+template <int NMAX>
+__device__ __forceinline__ void stored1d_lookup(const double* __restrict__ tab, long long atom_off, const int32_t (&lo)[3],
+                                                const int32_t (&hi)[3], int d, int i, int numax, bool valid, double (&out)[NMAX])
+{
+    const int M = numax + 1;
+    long long base = atom_off;
+    if (d >= 1) base += (long long)(hi[0] - lo[0] + 1) * M;
+    if (d >= 2) base += (long long)(hi[1] - lo[1] + 1) * M;
+    const double* row = tab + base + (long long)(i - lo[d]) * M;
+#pragma unroll
+    for (int n = 0; n < NMAX; ++n) out[n] = (valid && n <= numax) ? __ldg(row + n) : 0.0;
+}
+
 // unwrapped index -> displacement from the atom, written as the paper's grid convention x_i = i*h
 // (no FMA contraction, so box-edge values match a plain evaluation)
 __device__ __forceinline__ double displacement(int i, double h, double pos) { return __dsub_rn(__dmul_rn((double)i, h), pos); }

@@ -112,7 +112,17 @@ struct sho_tables {
     int32_t* d_seg_atom;                   // K segments (atom, first box plane) = the CTAs of the stored kernel
     int32_t* d_seg_qz0;
     int32_t nseg;
+    int* d_turn;                           // [turn_count] turnstile counters of sho_project_stored (256 column groups per atom)
+    size_t turn_count;
     std::vector<int64_t> atom_off;
+    size_t bytes;
+};
+
+struct sho_tables1d {
+    const sho_plan* plan;
+    uint64_t plan_serial;
+    double* d_data;                        // per atom: x rows, y rows, z rows; M = numax + 1 doubles per box index
+    long long* d_atom_off;                 // [natoms] first element of the atom
     size_t bytes;
 };
 
@@ -125,8 +135,12 @@ inline bool is_complex(sho_dtype t) { return t == SHO_C128 || t == SHO_C64; }
 
 // launchers (defined next to their kernels)
 // cnb: bands per atom in the coefficient array when the launch covers a chunk of a wider array (0: nbands)
-sho_status launch_project(const sho_plan* p, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb = 0);
-sho_status launch_add(const sho_plan* p, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb = 0);
+sho_status launch_project(const sho_plan* p, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb = 0,
+                          const sho_tables1d* t1 = nullptr);
+sho_status launch_add(const sho_plan* p, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb = 0,
+                      const sho_tables1d* t1 = nullptr);
+sho_status tables1d_build(const sho_plan* p, sho_tables1d** out, size_t* bytes_needed, cudaStream_t s);
+sho_status launch_add_stored(const sho_plan* p, const sho_tables* t, const void* coeff, int nbands, void* psi, cudaStream_t s);
 sho_status launch_to_x_fastest(const sho_plan* p, const void* psi_bf, int nbands, int b0, int nb, void* psi_xf, cudaStream_t s);
 sho_status launch_from_x_fastest(const sho_plan* p, const void* psi_xf, int nbands, int b0, int nb, void* psi_bf, cudaStream_t s);
 sho_status launch_dmul(const sho_plan* p, const double* dmat, const void* cin, int nbands, void* cout, cudaStream_t s);

@@ -41,6 +41,8 @@ struct ProjParams {
     const AtomDev* atoms;
     const int32_t* order;
     const uint32_t* nxyz;
+    const double* tab1d;       // stored 1D tables (sho_project_stored1d), or null: sample on the fly
+    const long long* tab1d_off;
     int32_t nbands;
     int32_t cnb;               // bands per atom in the coefficient array (>= nbands: a chunk of a wider array)
     int32_t n_work_atoms;      // atoms with a non-empty box (first entries of order[])
@@ -185,7 +187,8 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
             const int ix = xs0 + CWX * (k - (k > kdup ? 1 : 0)) + r;
             const bool valid = ix >= at.lo[0] && ix <= at.hi[0] &&
                                (kdup == INT_MAX || (k < krot ? ix < xB : ix >= xB));
-            hermite_gauss<NV>(displacement(ix, p.g.h, at.pos[0]), at, p.g.hnorm, numax, valid, v);
+            if (p.tab1d) stored1d_lookup<NV>(p.tab1d, p.tab1d_off[a], at.lo, at.hi, 0, ix, numax, valid, v);
+            else hermite_gauss<NV>(displacement(ix, p.g.h, at.pos[0]), at, p.g.hnorm, numax, valid, v);
             // A fragments [step][mt][e / 2][lane = 4 nx + t][e & 1]: 16-byte loads, lanes 16 bytes apart (no bank conflicts)
 #pragma unroll
             for (int n = 0; n < MP; ++n)
@@ -196,7 +199,8 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
             int iy = at.lo[1] + pr;
             const bool valid = iy <= at.hi[1];
             if (!valid) iy = at.hi[1];
-            hermite_gauss<NV>(displacement(iy, p.g.h, at.pos[1]), at, p.g.hnorm, numax, valid, v);
+            if (p.tab1d) stored1d_lookup<NV>(p.tab1d, p.tab1d_off[a], at.lo, at.hi, 1, iy, numax, valid, v);
+            else hermite_gauss<NV>(displacement(iy, p.g.h, at.pos[1]), at, p.g.hnorm, numax, valid, v);
             const int yb = pr >> 3, r = pr & 7, tt = r >> 1, s = r & 1;          // row r of the block = 2 t + s
 #pragma unroll
             for (int n = 0; n < MP; ++n) fy[(((size_t)yb * 2 + s) * MT + (n >> 3)) * 32 + (n & 7) * 4 + tt] = v[n];
@@ -212,7 +216,8 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
         } else {
             const int zi = it - nx_items - ny_items;
             const int iz = at.lo[2] + zi;
-            hermite_gauss<NV>(displacement(iz, p.g.h, at.pos[2]), at, p.g.hnorm, numax, true, v);
+            if (p.tab1d) stored1d_lookup<NV>(p.tab1d, p.tab1d_off[a], at.lo, at.hi, 2, iz, numax, true, v);
+            else hermite_gauss<NV>(displacement(iz, p.g.h, at.pos[2]), at, p.g.hnorm, numax, true, v);
 #pragma unroll
             for (int n = 0; n < NV; ++n) fz[(size_t)zi * NV + n] = v[n];
             if (CPLX) {
@@ -575,7 +580,7 @@ __global__ void sho_zero_empty_kernel(T* coeff, const int32_t* order, int first,
 }
 
 template <int MT, int R, int DT, int G>
-static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb)
+static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb, const sho_tables1d* t1)
 {
     using S = ProjSmem<MT, R, DT>;
     constexpr bool CPLX = Elem<DT>::cplx;
@@ -584,6 +589,7 @@ static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void
     p.g = pl->g;
     p.psi = psi; p.coeff = coeff;
     p.atoms = pl->d_atoms; p.order = pl->d_order; p.nxyz = pl->d_nxyz;
+    p.tab1d = t1 ? t1->d_data : nullptr; p.tab1d_off = t1 ? t1->d_atom_off : nullptr;
     p.nbands = nbands;
     p.cnb = cnb;
     p.n_work_atoms = pl->n_nonempty;
@@ -621,33 +627,33 @@ static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void
 }
 
 template <int DT, int G>
-static sho_status launch_mg(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb)
+static sho_status launch_mg(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb, const sho_tables1d* t1)
 {
     // numax + 1 functions per axis: <= 8 one MMA row tile; 9, 10 one tile + 2 DFMA rows; more: two tiles
     const int M = pl->g.numax + 1;
-    if (M <= 8) return launch_t<1, 0, DT, G>(pl, psi, nbands, coeff, s, cnb);
-    if (M <= 10) return launch_t<1, 2, DT, G>(pl, psi, nbands, coeff, s, cnb);
-    return launch_t<2, 0, DT, G>(pl, psi, nbands, coeff, s, cnb);
+    if (M <= 8) return launch_t<1, 0, DT, G>(pl, psi, nbands, coeff, s, cnb, t1);
+    if (M <= 10) return launch_t<1, 2, DT, G>(pl, psi, nbands, coeff, s, cnb, t1);
+    return launch_t<2, 0, DT, G>(pl, psi, nbands, coeff, s, cnb, t1);
 }
 
 template <int DT>
-static sho_status launch_m(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb)
+static sho_status launch_m(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb, const sho_tables1d* t1)
 {
     // Loads are issued kProjG = 2 steps at a time (longer prefetch distance); a row block with an odd number of
     // steps then wastes one.  Real data has few, long steps (16 or 32 columns): when more than 6 % of them would
     // be lost, issue them one by one (cfg 3: 4-5 steps per row block, 1.90 vs 2.03 ms; cfg 4: 8, 15.5 vs 16.1 ms).
-    if (!Elem<DT>::cplx && pl->proj_odd_steps > 0.06) return launch_mg<DT, 1>(pl, psi, nbands, coeff, s, cnb);
-    return launch_mg<DT, kProjG>(pl, psi, nbands, coeff, s, cnb);
+    if (!Elem<DT>::cplx && pl->proj_odd_steps > 0.06) return launch_mg<DT, 1>(pl, psi, nbands, coeff, s, cnb, t1);
+    return launch_mg<DT, kProjG>(pl, psi, nbands, coeff, s, cnb, t1);
 }
 
-sho_status launch_project(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb)
+sho_status launch_project(const sho_plan* pl, const void* psi, int nbands, void* coeff, cudaStream_t s, int cnb, const sho_tables1d* t1)
 {
     if (cnb <= 0) cnb = nbands;
     switch (pl->dtype) {
-        case SHO_R64:  return launch_m<SHO_R64>(pl, psi, nbands, coeff, s, cnb);
-        case SHO_C128: return launch_m<SHO_C128>(pl, psi, nbands, coeff, s, cnb);
-        case SHO_R32:  return launch_m<SHO_R32>(pl, psi, nbands, coeff, s, cnb);
-        case SHO_C64:  return launch_m<SHO_C64>(pl, psi, nbands, coeff, s, cnb);
+        case SHO_R64:  return launch_m<SHO_R64>(pl, psi, nbands, coeff, s, cnb, t1);
+        case SHO_C128: return launch_m<SHO_C128>(pl, psi, nbands, coeff, s, cnb, t1);
+        case SHO_R32:  return launch_m<SHO_R32>(pl, psi, nbands, coeff, s, cnb, t1);
+        case SHO_C64:  return launch_m<SHO_C64>(pl, psi, nbands, coeff, s, cnb, t1);
     }
     set_error("sho_project: bad dtype");
     return SHO_ERR_INVALID_ARG;

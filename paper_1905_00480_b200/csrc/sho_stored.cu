@@ -15,7 +15,7 @@
 namespace sho {
 
 constexpr int kStoWarps = 8;
-constexpr int kStoPlanes = 8;       // z planes of the box per CTA (K split; partial sums meet by atomicAdd)
+constexpr int kStoPlanes = 8;       // z planes of the box per CTA (K split; the partial sums are added in segment order)
 constexpr int kStoCols = 32;        // real columns (bands x re/im) per CTA
 constexpr int kStoKC = 32;          // K steps staged in shared memory at a time (128 points)
 constexpr int kStoKStride = (kStoCols / 8) * 32 + 4;   // padded stride of one K step in shared memory
@@ -75,6 +75,8 @@ struct StoParams {
     int32_t nseg;
     int32_t nbands;
     long long band_stride;
+    int* turn;                   // [natoms][ngroups] turnstile of the stored projection's K segments
+    int32_t ngroups;
 };
 
 template <int MTW, int DT>
@@ -177,9 +179,23 @@ __global__ void __launch_bounds__(kStoWarps * 32, 2) sho_project_stored_kernel(c
             }
         }
     }
-    // ---- partial sums of this K segment meet in c by atomicAdd (c was zeroed by the launcher) ----
+    // ---- the partial sums of the K segments of one (atom, column group) are added to c in segment order: segment k
+    // waits until k - 1 has published its sum (a turnstile counter per (atom, group), zeroed by the launcher; the CTA
+    // of segment k - 1 has the block index before this one, so it is already running or done), then does a plain
+    // read-modify-write.  Fixed summation order, no atomics on the data: bit-reproducible.  (fp32 data: each
+    // segment's sum is rounded to fp32 when it is added -- the one place where this baseline does not round once.)
     const double h3 = p.g.h * p.g.h * p.g.h;
     real_t* cout = reinterpret_cast<real_t*>(p.coeff);
+    const int kseg = qz0 / kStoPlanes;
+    int* turn = p.turn + (size_t)a * p.ngroups + bg;
+    __syncthreads();
+    if (kseg > 0) {
+        if (tid == 0) {
+            while (atomicAdd(turn, 0) != kseg) __nanosleep(64);
+            __threadfence();
+        }
+        __syncthreads();
+    }
 #pragma unroll
     for (int i = 0; i < MTW; ++i) {
         const int n = 8 * (warp + i * kStoWarps) + q;
@@ -190,11 +206,17 @@ __global__ void __launch_bounds__(kStoWarps * 32, 2) sho_project_stored_kernel(c
                 for (int s = 0; s < 2; ++s) {
                     const int col = 8 * j + 2 * t + s;
                     const int bl = col / P, pp = col - bl * P;
-                    if (bl < nbl)
-                        atomicAdd(cout + (((size_t)a * p.nbands + band0 + bl) * p.g.nsho + n) * P + pp, (real_t)(h3 * D[i][j][s]));
+                    if (bl < nbl) {
+                        real_t* o = cout + (((size_t)a * p.nbands + band0 + bl) * p.g.nsho + n) * P + pp;
+                        const double prev = (kseg > 0) ? (double)__ldcg(o) : 0.0;
+                        *o = (real_t)(prev + h3 * D[i][j][s]);
+                    }
                 }
         }
     }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) atomicExch(turn, kseg + 1);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -238,10 +260,10 @@ sho_status tables_build(const sho_plan* pl, sho_tables** out, size_t* bytes_need
     }
     sho_tables* t = new (std::nothrow) sho_tables();
     if (!t) { set_error("sho_tables_build: host allocation failed"); return SHO_ERR_OOM; }
-    t->plan = pl; t->plan_serial = pl->serial; t->d_data = nullptr; t->d_atom_off = nullptr; t->d_seg_atom = nullptr; t->d_seg_qz0 = nullptr;
+    t->plan = pl; t->plan_serial = pl->serial; t->d_turn = nullptr; t->turn_count = (size_t)std::max<size_t>(pl->atoms.size(), 1) * 256; t->d_data = nullptr; t->d_atom_off = nullptr; t->d_seg_atom = nullptr; t->d_seg_qz0 = nullptr;
     t->atom_off = off; t->bytes = *bytes_needed; t->nseg = (int32_t)seg_atom.size();
     int32_t *d_pa = nullptr, *d_pq = nullptr;
-    auto fail = [&](sho_status st) { cudaFree(d_pa); cudaFree(d_pq); cudaFree(t->d_seg_atom); cudaFree(t->d_seg_qz0);
+    auto fail = [&](sho_status st) { cudaFree(d_pa); cudaFree(d_pq); cudaFree(t->d_turn); cudaFree(t->d_seg_atom); cudaFree(t->d_seg_qz0);
                                      cudaFree(t->d_data); cudaFree(t->d_atom_off); delete t; return st; };
     auto up = [&](void** dst, const void* src, size_t bytes) -> cudaError_t {
         cudaError_t ee = cudaMalloc(dst, std::max<size_t>(bytes, 16));
@@ -253,6 +275,7 @@ sho_status tables_build(const sho_plan* pl, sho_tables** out, size_t* bytes_need
         set_error("sho_tables_build: cudaMalloc of %zu bytes failed", t->bytes);
         return fail(SHO_ERR_OOM);
     }
+    if ((e = cudaMalloc(&t->d_turn, t->turn_count * sizeof(int))) != cudaSuccess) return fail(cuda_fail(e, "sho_tables_build: turnstile"));
     if ((e = up((void**)&t->d_atom_off, off.data(), off.size() * 8)) != cudaSuccess ||
         (e = up((void**)&t->d_seg_atom, seg_atom.data(), seg_atom.size() * 4)) != cudaSuccess ||
         (e = up((void**)&t->d_seg_qz0, seg_qz0.data(), seg_qz0.size() * 4)) != cudaSuccess ||
@@ -286,9 +309,17 @@ static sho_status launch_t(const sho_plan* pl, const sho_tables* tb, const void*
     p.atoms = pl->d_atoms; p.atom_off = tb->d_atom_off; p.seg_atom = tb->d_seg_atom; p.seg_qz0 = tb->d_seg_qz0;
     p.nseg = tb->nseg; p.nbands = nbands;
     p.band_stride = (long long)pl->g.ng[0] * pl->g.ng[1] * pl->g.ng[2];
-    cudaError_t e = cudaMemsetAsync(coeff, 0, (size_t)pl->g.natoms * nbands * pl->g.nsho * elem_size(pl->dtype), s);
-    if (e != cudaSuccess) return cuda_fail(e, "sho_project_stored: memset");
     const int ngroups = (nbands * P + kStoCols - 1) / kStoCols;
+    if ((size_t)pl->g.natoms * ngroups > tb->turn_count) {
+        set_error("sho_project_stored: %d bands need more turnstile counters than the tables hold (at most %zu column groups per atom)",
+                  nbands, pl->g.natoms ? tb->turn_count / (size_t)pl->g.natoms : (size_t)0);
+        return SHO_ERR_UNSUPPORTED;
+    }
+    // atoms with an empty box have no segment: their coefficients are the zeros written here
+    cudaError_t e = cudaMemsetAsync(coeff, 0, (size_t)pl->g.natoms * nbands * pl->g.nsho * elem_size(pl->dtype), s);
+    if (e == cudaSuccess) e = cudaMemsetAsync(tb->d_turn, 0, (size_t)pl->g.natoms * ngroups * sizeof(int), s);
+    if (e != cudaSuccess) return cuda_fail(e, "sho_project_stored: memset");
+    p.turn = tb->d_turn; p.ngroups = ngroups;
     const long long nblocks = (long long)tb->nseg * ngroups;
     if (nblocks > 0x7fffffffLL) { set_error("sho_project_stored: grid too large"); return SHO_ERR_UNSUPPORTED; }
     if (nblocks > 0) {
@@ -320,6 +351,180 @@ sho_status launch_project_stored(const sho_plan* pl, const sho_tables* tb, const
     }
     set_error("sho_project_stored: bad dtype");
     return SHO_ERR_INVALID_ARG;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Stored add-back (the paper's "USUadd", tab. 1): the expansion of step (3), PAPER.md:190,
+//     psi_b(r) += conj(w(r)) sum_n T[a][n][r] c[a][b][n]
+// reading the same pre-sampled 3D tables.  Per (atom, 8 box planes, 32 real columns) a GEMM M = box points,
+// K = n (N_SHO), N = columns on the FP64 tensor cores; the table fragments are read with the transposed lane
+// mapping (lane (q,t) takes T[n = 4 ks + t][point 8 pt + q]: two runs of 128 contiguous bytes per warp).  The boxes
+// of different atoms overlap and this baseline does what a stored-projector code does: it adds its results to psi
+// with atomicAdd (so, unlike sho_add, it is not bit-reproducible).
+template <int DT>
+__global__ void __launch_bounds__(kStoWarps * 32, 2) sho_add_stored_kernel(const StoParams p)
+{
+    using E = Elem<DT>;
+    using real_t = typename E::real_t;
+    constexpr bool CPLX = E::cplx;
+    constexpr int P = CPLX ? 2 : 1;
+    constexpr int NT = kStoCols / 8;
+    extern __shared__ __align__(16) double cs[];          // [ks][nt][32] B fragments: lane (q,t) holds c[n = 4 ks + t][col 8 nt + q]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int q = lane >> 2, t = lane & 3;
+    const int seg = blockIdx.x % p.nseg, bg = blockIdx.x / p.nseg;
+    const int a = p.seg_atom[seg], qz0 = p.seg_qz0[seg];
+    const AtomDev at = p.atoms[a];
+    const int Nx = p.g.ng[0], Ny = p.g.ng[1], Nz = p.g.ng[2];
+    const int nxl = at.hi[0] - at.lo[0] + 1, nyl = at.hi[1] - at.lo[1] + 1, nzl = at.hi[2] - at.lo[2] + 1;
+    const int npl = nxl * nyl, KP = (npl + 3) >> 2, MTILES = sto_mtiles(p.g.nsho);
+    const int n = p.g.nsho, KS = (n + 3) >> 2;
+    const int band0 = bg * (kStoCols / P);
+    const int ncols = min(kStoCols, (p.nbands - band0) * P);
+    const real_t* tab = reinterpret_cast<const real_t*>(p.data) + p.atom_off[a];
+    const real_t* cin = reinterpret_cast<const real_t*>(p.coeff) + ((size_t)a * p.nbands + band0) * n * P;
+    real_t* psi = reinterpret_cast<real_t*>(const_cast<void*>(p.psi));
+    for (int e = tid; e < KS * 4 * kStoCols; e += blockDim.x) {
+        const int j = e % (KS * 4), cl = e / (KS * 4);
+        double v = 0.0;
+        if (j < n && cl < ncols) v = (double)cin[((size_t)(cl / P) * n + j) * P + (cl % P)];
+        cs[((j >> 2) * NT + (cl >> 3)) * 32 + (cl & 7) * 4 + (j & 3)] = v;
+    }
+    __syncthreads();
+    const int qz1 = min(qz0 + kStoPlanes, nzl);
+    const int NPT = (npl + 7) >> 3;                          // groups of 8 points per plane
+    for (int work = warp; work < (qz1 - qz0) * NPT; work += kStoWarps) {
+        const int qz = qz0 + work / NPT, pt = work % NPT;
+        const real_t* tpl = tab + (size_t)qz * KP * MTILES * 32;
+        double D[NT][2];
+#pragma unroll
+        for (int j = 0; j < NT; ++j) D[j][0] = D[j][1] = 0.0;
+        // A[point 8 pt + q][n = 4 ks + t] = T[n][point]: element (n, r) of the plane sits at ((r >> 2) MTILES + (n >> 3)) 32 + (n & 7) 4 + (r & 3)
+        const int r = 8 * pt + q;
+        const size_t rbase = (size_t)(r >> 2) * MTILES * 32 + (r & 3);
+        const bool rin = (r >> 2) < KP;
+#pragma unroll 4
+        for (int ks = 0; ks < KS; ++ks) {
+            const int nn = 4 * ks + t;
+            const double av = (rin && nn < 8 * MTILES) ? (double)__ldcs(tpl + rbase + (size_t)(nn >> 3) * 32 + (nn & 7) * 4) : 0.0;
+#pragma unroll
+            for (int j = 0; j < NT; ++j) dmma(D[j][0], D[j][1], av, cs[(ks * NT + j) * 32 + lane]);
+        }
+        // this lane holds point r (row q) x columns 8 j + 2 t, 2 t + 1
+        if (r < npl) {
+            const int iz = at.lo[2] + qz;
+            const int mz = p.g.periodic[2] ? floordiv(iz, Nz) : 0;
+            const int qy = r / nxl, qx = r - qy * nxl;
+            const int ix = at.lo[0] + qx, iy = at.lo[1] + qy;
+            const int mx = p.g.periodic[0] ? floordiv(ix, Nx) : 0, my = p.g.periodic[1] ? floordiv(iy, Ny) : 0;
+            const size_t jpt = ((size_t)(iz - mz * Nz) * Ny + (iy - my * Ny)) * Nx + (ix - mx * Nx);
+            double cw = 1.0, sw = 0.0;
+            if (CPLX && p.g.has_phase && (mx | my | mz))
+                sincospi(-2.0 * (p.g.kfrac[0] * mx + p.g.kfrac[1] * my + p.g.kfrac[2] * mz), &sw, &cw);      // conj(w)
+#pragma unroll
+            for (int j = 0; j < NT; ++j) {
+                const int col = 8 * j + 2 * t;
+                if (col >= ncols) continue;
+                if (CPLX) {      // columns (2t, 2t+1) = (re, im) of one band
+                    real_t* o = psi + ((size_t)(band0 + col / 2) * p.band_stride + jpt) * 2;
+                    atomicAdd(o, (real_t)(D[j][0] * cw - D[j][1] * sw));
+                    atomicAdd(o + 1, (real_t)(D[j][0] * sw + D[j][1] * cw));
+                } else {
+                    atomicAdd(psi + (size_t)(band0 + col) * p.band_stride + jpt, (real_t)D[j][0]);
+                    if (col + 1 < ncols) atomicAdd(psi + (size_t)(band0 + col + 1) * p.band_stride + jpt, (real_t)D[j][1]);
+                }
+            }
+        }
+    }
+}
+
+template <int DT>
+static sho_status launch_add_t(const sho_plan* pl, const sho_tables* tb, const void* coeff, int nbands, void* psi, cudaStream_t s)
+{
+    constexpr int P = Elem<DT>::cplx ? 2 : 1;
+    StoParams p;
+    p.g = pl->g; p.psi = psi; p.coeff = const_cast<void*>(coeff); p.data = tb->d_data;
+    p.atoms = pl->d_atoms; p.atom_off = tb->d_atom_off; p.seg_atom = tb->d_seg_atom; p.seg_qz0 = tb->d_seg_qz0;
+    p.nseg = tb->nseg; p.nbands = nbands; p.turn = nullptr; p.ngroups = 0;
+    p.band_stride = (long long)pl->g.ng[0] * pl->g.ng[1] * pl->g.ng[2];
+    const int ngroups = (nbands * P + kStoCols - 1) / kStoCols;
+    const long long nblocks = (long long)tb->nseg * ngroups;
+    if (nblocks > 0x7fffffffLL) { set_error("sho_add_stored: grid too large"); return SHO_ERR_UNSUPPORTED; }
+    if (nblocks == 0) return SHO_OK;
+    const size_t smem = (size_t)((pl->g.nsho + 3) / 4) * (kStoCols / 8) * 32 * sizeof(double);
+    auto kern = sho_add_stored_kernel<DT>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(add_stored)");
+    kern<<<(unsigned)nblocks, kStoWarps * 32, smem, s>>>(p);
+    if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "launch sho_add_stored_kernel");
+    return SHO_OK;
+}
+
+sho_status launch_add_stored(const sho_plan* pl, const sho_tables* tb, const void* coeff, int nbands, void* psi, cudaStream_t s)
+{
+    switch (pl->dtype) {
+        case SHO_R64:  return launch_add_t<SHO_R64>(pl, tb, coeff, nbands, psi, s);
+        case SHO_C128: return launch_add_t<SHO_C128>(pl, tb, coeff, nbands, psi, s);
+        case SHO_R32:  return launch_add_t<SHO_R32>(pl, tb, coeff, nbands, psi, s);
+        case SHO_C64:  return launch_add_t<SHO_C64>(pl, tb, coeff, nbands, psi, s);
+    }
+    set_error("sho_add_stored: bad dtype");
+    return SHO_ERR_INVALID_ARG;
+}
+
+// ------------------------------------------------------------------------------------------------
+// stored 1D tables (f3): the separable scheme with its factor matrices read from memory (sho_device.cuh::stored1d_lookup)
+__global__ void sho_tables1d_kernel(GridDev g, const AtomDev* atoms, const long long* atom_off, int natoms, double* data)
+{
+    const int a = blockIdx.x;
+    const AtomDev at = atoms[a];
+    const int M = g.numax + 1;
+    const int n0 = max(at.hi[0] - at.lo[0] + 1, 0), n1 = max(at.hi[1] - at.lo[1] + 1, 0), n2 = max(at.hi[2] - at.lo[2] + 1, 0);
+    if (n0 == 0 || n1 == 0 || n2 == 0) return;
+    for (int it = threadIdx.x; it < n0 + n1 + n2; it += blockDim.x) {
+        const int d = it < n0 ? 0 : it < n0 + n1 ? 1 : 2;
+        const int i = at.lo[d] + (d == 0 ? it : d == 1 ? it - n0 : it - n0 - n1);
+        double v[SHO_NUMAX_MAX + 1];
+        hermite_gauss<SHO_NUMAX_MAX + 1>(displacement(i, g.h, at.pos[d]), at, g.hnorm, g.numax, true, v);
+        double* dst = data + atom_off[a] + (size_t)it * M;
+        for (int n = 0; n < M; ++n) dst[n] = v[n];
+    }
+    (void)natoms;
+}
+
+sho_status tables1d_build(const sho_plan* pl, sho_tables1d** out, size_t* bytes_needed, cudaStream_t s)
+{
+    const int M = pl->g.numax + 1;
+    std::vector<long long> off(pl->atoms.size() + 1, 0);
+    for (size_t a = 0; a < pl->atoms.size(); ++a) {
+        const AtomDev& at = pl->atoms[a];
+        long long n = 0;
+        if (at.hi[0] >= at.lo[0] && at.hi[1] >= at.lo[1] && at.hi[2] >= at.lo[2])
+            n = (long long)((at.hi[0] - at.lo[0] + 1) + (at.hi[1] - at.lo[1] + 1) + (at.hi[2] - at.lo[2] + 1)) * M;
+        off[a + 1] = off[a] + n;
+    }
+    *bytes_needed = (size_t)off.back() * sizeof(double);
+    if (!out) return SHO_OK;
+    *out = nullptr;
+    sho_tables1d* t = new (std::nothrow) sho_tables1d();
+    if (!t) { set_error("sho_tables1d_build: host allocation failed"); return SHO_ERR_OOM; }
+    t->plan = pl; t->plan_serial = pl->serial; t->d_data = nullptr; t->d_atom_off = nullptr; t->bytes = *bytes_needed;
+    cudaError_t e = cudaMalloc(&t->d_data, std::max<size_t>(t->bytes, 16));
+    if (e == cudaSuccess) e = cudaMalloc(&t->d_atom_off, off.size() * sizeof(long long));
+    if (e == cudaSuccess) e = cudaMemcpy(t->d_atom_off, off.data(), off.size() * sizeof(long long), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(t->d_data); cudaFree(t->d_atom_off); delete t;
+        set_error("sho_tables1d_build: cannot allocate %zu bytes", *bytes_needed);
+        return SHO_ERR_OOM;
+    }
+    if (!pl->atoms.empty()) {
+        sho_tables1d_kernel<<<(unsigned)pl->atoms.size(), 128, 0, s>>>(pl->g, pl->d_atoms, t->d_atom_off, (int)pl->atoms.size(), t->d_data);
+        if ((e = cudaGetLastError()) == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) { cudaFree(t->d_data); cudaFree(t->d_atom_off); delete t; return cuda_fail(e, "sho_tables1d_build"); }
+    }
+    *out = t;
+    return SHO_OK;
 }
 
 }  // namespace sho

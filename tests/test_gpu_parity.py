@@ -101,6 +101,24 @@ def run_case(sho, w, stored=True, tol=None):
         scale = np.maximum(np.abs(ref).max(axis=(1, 2, 3)), 1e-300)
         err = (np.abs(got.astype(wide) - ref).max(axis=(1, 2, 3)) / scale).max()
         assert err <= tol, "add parity: max normalised error %.3e > %.1e" % (err, tol)
+        # ---- f3: the separable kernels on stored 1D tables, and the stored (3D tables) add-back ----
+        t1 = plan.tables1d()
+        c_1d = plan.project_stored1d(t1, d_psi)
+        d_psi1 = _dev(psi0)
+        plan.add_stored1d(t1, _dev(coeff), d_psi1)
+        torch.cuda.synchronize()
+        t1.close()
+        check_project(sho, w, psi, c_1d.cpu().numpy(), tol)
+        e1 = (np.abs(d_psi1.cpu().numpy().astype(wide) - ref).max(axis=(1, 2, 3)) / scale).max()
+        assert e1 <= tol, "stored-1D add parity: %.3e > %.1e" % (e1, tol)
+        if stored:
+            tb = plan.tables()
+            d_psi2 = _dev(psi0)
+            plan.add_stored(tb, _dev(coeff), d_psi2)
+            torch.cuda.synchronize()
+            tb.close()
+            e2 = (np.abs(d_psi2.cpu().numpy().astype(wide) - ref).max(axis=(1, 2, 3)) / scale).max()
+            assert e2 <= tol, "stored add parity: %.3e > %.1e" % (e2, tol)
         return e_prj, float(err)
     finally:
         plan.close()
@@ -472,6 +490,20 @@ def test_project_and_add_are_bit_reproducible_under_load(sho, k):
             ref = cur
         assert torch.equal(ref[0], cur[0]) and torch.equal(ref[1], cur[1]), "run %d differs bit-wise from run 0" % it
     plan.close()
+
+
+def test_stored_projection_is_bit_reproducible(sho):
+    # its K segments are added in a fixed order through a turnstile, not by atomicAdd
+    import torch
+    w = workloads.make(3, size="small")
+    plan = sho.plan_for(w)
+    psi = _dev(w.psi())
+    tb = plan.tables()
+    outs = [plan.project_stored(tb, psi).clone() for _ in range(4)]
+    torch.cuda.synchronize()
+    tb.close()
+    plan.close()
+    assert all(torch.equal(outs[0], o) for o in outs[1:])
 
 
 def test_host_buffer_entry_points(sho):
