@@ -133,6 +133,25 @@ sho_status sho_dmul(const sho_plan* plan, const double* dmat, const void* coeff_
                     void* cuda_stream);
 
 /*
+ * Coefficients in the spherical representation (nr, l, m) (f4; eq. (10)-(11)): the unitary
+ * transform U between the Cartesian eigenstates Psi_{nx ny nz} and the spherical ones Psi_{nr l m} = R_{nr l}(r/sigma)
+ * Y_lm (eq. (7)-(8)).  The paper gives no formula for its elements; sho_umatrix evaluates the overlap
+ * integrals exactly (host code, Gauss-Hermite).  Conventions (readings A17-A19): spherical index ordered by
+ * nu = l + 2 nr ascending, then nr ascending (l descending), then m = -l..l; REAL spherical harmonics with positive
+ * factors (Y_1,-1 ~ y, Y_10 ~ z, Y_11 ~ x); R_{nr l} > 0 at the origin.  U is real orthogonal and vanishes outside
+ * the nu-blocks (eq. (11)).
+ *   sho_rlm_index  position of (nr, l, m) in that order, -1 if not in the basis
+ *   sho_umatrix    u HOST [N_SHO][N_SHO] row-major: u[rlm][sho_index(nx,ny,nz)]
+ *   sho_transform  coeff_out[a][b][i] = sum_j umat[i][j] coeff_in[a][b][j] for every atom and band (umat DEVICE fp64
+ *                  [N_SHO][N_SHO]; pass U for Cartesian -> spherical, its transpose for the way back; coeff_out may be
+ *                  coeff_in).  Runs the batched tensor-core GEMM of sho_dmul with one shared matrix.
+ */
+int sho_rlm_index(int nr, int l, int m, int numax);
+sho_status sho_umatrix(int numax, double* u);
+sho_status sho_transform(const sho_plan* plan, const double* umat, const void* coeff_in, int32_t nbands, void* coeff_out,
+                         void* cuda_stream);
+
+/*
  * The three steps of PAPER.md:187-190 in one call: c = project(psi); d = D c; psi += add(d), on one stream.
  * psi DEVICE in/out, coeff_work DEVICE [natoms][nbands][N_SHO] caller-owned scratch (holds d on return).
  */

@@ -19,3 +19,4 @@ from .sho_oracle import (  # noqa: F401
     dmul,
     num_threads,
 )
+from .sho_umatrix import rlm_index, umatrix  # noqa: F401,E402

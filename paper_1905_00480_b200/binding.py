@@ -85,6 +85,9 @@ def lib():
     L.sho_project_host.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
     L.sho_add_host.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
     L.sho_measure_fp64_peak.argtypes = [C.c_int32, _f64p]
+    L.sho_rlm_index.argtypes = [C.c_int] * 4; L.sho_rlm_index.restype = C.c_int
+    L.sho_umatrix.argtypes = [C.c_int, _f64p]
+    L.sho_transform.argtypes = [_vp, _vp, _vp, C.c_int32, _vp, _vp]
     L.sho_add_stored.argtypes = [_vp, _vp, _vp, C.c_int32, _vp, _vp]
     L.sho_tables1d_build.argtypes = [_vp, C.POINTER(_vp), C.POINTER(C.c_size_t), _vp]
     L.sho_tables1d_destroy.argtypes = [_vp]
@@ -97,7 +100,7 @@ def lib():
     L.sho_apply_host.argtypes = [_vp, _vp, _vp, C.c_int32, _vp]
     for name in DECLARED_SYMBOLS:
         fn = getattr(L, name)   # AttributeError here = header and library disagree
-        if name not in ("sho_status_string", "sho_last_error"):
+        if name not in ("sho_status_string", "sho_last_error", "sho_nsho", "sho_index", "sho_rlm_index"):
             fn.restype = C.c_int
     _lib = L
     return L
@@ -114,6 +117,20 @@ def nsho(numax: int) -> int:
 
 def index(nx: int, ny: int, nz: int, numax: int) -> int:
     return int(lib().sho_index(int(nx), int(ny), int(nz), int(numax)))
+
+
+def rlm_index(nr: int, l: int, m: int, numax: int) -> int:
+    return int(lib().sho_rlm_index(int(nr), int(l), int(m), int(numax)))
+
+
+def umatrix(numax: int) -> np.ndarray:
+    """U[rlm_index][index] between Cartesian and spherical SHO states (sho_umatrix; host computation)."""
+    n = nsho(numax)
+    if n < 0:
+        raise ValueError("numax out of range")
+    out = np.zeros((n, n), dtype=np.float64)
+    _check(lib().sho_umatrix(int(numax), out.ctypes.data_as(_f64p)), "sho_umatrix")
+    return out
 
 
 def _torch():
@@ -280,6 +297,20 @@ class Plan:
             out = self.new_coeff(nb, coeff.device)
         self._check_coeff(out, nb, "sho_dmul")
         _check(lib().sho_dmul(self._h, dmat.data_ptr(), coeff.data_ptr(), nb, out.data_ptr(), _stream_handle(stream)), "sho_dmul")
+        return out
+
+    def transform(self, umat, coeff, out=None, stream=None):
+        """out[a][b][i] = sum_j umat[i][j] coeff[a][b][j]: one [N_SHO][N_SHO] matrix for all atoms (sho_transform)."""
+        torch = _torch()
+        nb = int(coeff.shape[1])
+        self._check_coeff(coeff, nb, "sho_transform")
+        if not (isinstance(umat, torch.Tensor) and umat.is_cuda and umat.is_contiguous() and umat.dtype == torch.float64
+                and tuple(umat.shape) == (self.nsho, self.nsho) and umat.device.index == self.device):
+            raise ValueError("sho_transform: umat must be a contiguous float64 CUDA tensor [N_SHO][N_SHO] on the plan's device")
+        if out is None:
+            out = self.new_coeff(nb, coeff.device)
+        self._check_coeff(out, nb, "sho_transform")
+        _check(lib().sho_transform(self._h, umat.data_ptr(), coeff.data_ptr(), nb, out.data_ptr(), _stream_handle(stream)), "sho_transform")
         return out
 
     def apply(self, dmat, psi, coeff_work=None, stream=None):
@@ -458,6 +489,10 @@ def sho_project_bf(plan: Plan, psi_bf, coeff=None, work=None, stream=None):
 
 def sho_add_bf(plan: Plan, coeff, psi_bf, work=None, stream=None):
     return plan.add_bf(coeff, psi_bf, work, stream)
+
+
+def sho_transform(plan: Plan, umat, coeff, out=None, stream=None):
+    return plan.transform(umat, coeff, out, stream)
 
 
 def sho_dmul(plan: Plan, dmat, coeff, out=None, stream=None):

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libsho.so")
-SOURCES = ("sho_api.cu", "sho_project.cu", "sho_add.cu", "sho_stored.cu", "sho_dmul.cu", "sho_layout.cu")
+SOURCES = ("sho_api.cu", "sho_project.cu", "sho_add.cu", "sho_stored.cu", "sho_dmul.cu", "sho_layout.cu", "sho_umat.cu")
 HEADERS = ("sho_internal.h", "sho_device.cuh")
 
 NVCC_FLAGS = [

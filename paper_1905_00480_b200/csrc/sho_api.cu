@@ -495,6 +495,16 @@ sho_status sho_dmul(const sho_plan* plan, const double* dmat, const void* coeff_
     return launch_dmul(plan, dmat, coeff_in, nbands, coeff_out, static_cast<cudaStream_t>(cuda_stream));
 }
 
+sho_status sho_transform(const sho_plan* plan, const double* umat, const void* coeff_in, int32_t nbands, void* coeff_out,
+                         void* cuda_stream)
+{
+    if (plan && plan->g.natoms == 0 && nbands > 0) return SHO_OK;
+    sho_status st = check_hot("sho_transform", plan, coeff_in, coeff_out, nbands);
+    if (st != SHO_OK) return st;
+    if (!umat) { set_error("sho_transform: null argument"); return SHO_ERR_INVALID_ARG; }
+    return launch_dmul(plan, umat, coeff_in, nbands, coeff_out, static_cast<cudaStream_t>(cuda_stream), true);
+}
+
 sho_status sho_apply(const sho_plan* plan, const double* dmat, void* psi, int32_t nbands, void* coeff_work, void* cuda_stream)
 {
     if (plan && plan->g.natoms == 0 && psi && nbands > 0) return SHO_OK;

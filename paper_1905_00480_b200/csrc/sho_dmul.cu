@@ -22,6 +22,7 @@ struct DmulParams {
     const void* cin;
     void* cout;
     int32_t nsho, nbands, natoms, ncolchunks;
+    long long dstride;         // doubles between the matrices of two atoms (0: one matrix for all atoms, sho_transform)
 };
 
 template <int DT>
@@ -49,7 +50,7 @@ __global__ void __launch_bounds__(kDmWarps * 32) sho_dmul_kernel(const DmulParam
         bs[((j >> 2) * NT + (cl >> 3)) * 32 + (cl & 7) * 4 + (j & 3)] = v;
     }
     __syncthreads();
-    const double* D = p.dmat + (size_t)a * n * n;
+    const double* D = p.dmat + (size_t)a * p.dstride;
     for (int mt = warp; mt < MT; mt += kDmWarps) {
         const int i = 8 * mt + q;
         const double* drow = D + (size_t)min(i, n - 1) * n;
@@ -76,13 +77,14 @@ __global__ void __launch_bounds__(kDmWarps * 32) sho_dmul_kernel(const DmulParam
 }
 
 template <int DT>
-static sho_status launch_t(const sho_plan* pl, const double* dmat, const void* cin, int nbands, void* cout, cudaStream_t s)
+static sho_status launch_t(const sho_plan* pl, const double* dmat, const void* cin, int nbands, void* cout, cudaStream_t s, bool shared)
 {
     constexpr int P = Elem<DT>::cplx ? 2 : 1;
     DmulParams p;
     p.dmat = dmat; p.cin = cin; p.cout = cout;
     p.nsho = pl->g.nsho; p.nbands = nbands; p.natoms = pl->g.natoms;
     p.ncolchunks = (nbands * P + kDmCols - 1) / kDmCols;
+    p.dstride = shared ? 0 : (long long)pl->g.nsho * pl->g.nsho;
     const long long nblocks = (long long)pl->g.natoms * p.ncolchunks;
     if (nblocks > 0x7fffffffLL) { set_error("sho_dmul: natoms*nbands too large"); return SHO_ERR_UNSUPPORTED; }
     if (nblocks == 0) return SHO_OK;
@@ -96,13 +98,13 @@ static sho_status launch_t(const sho_plan* pl, const double* dmat, const void* c
     return SHO_OK;
 }
 
-sho_status launch_dmul(const sho_plan* pl, const double* dmat, const void* cin, int nbands, void* cout, cudaStream_t s)
+sho_status launch_dmul(const sho_plan* pl, const double* dmat, const void* cin, int nbands, void* cout, cudaStream_t s, bool shared)
 {
     switch (pl->dtype) {
-        case SHO_R64:  return launch_t<SHO_R64>(pl, dmat, cin, nbands, cout, s);
-        case SHO_C128: return launch_t<SHO_C128>(pl, dmat, cin, nbands, cout, s);
-        case SHO_R32:  return launch_t<SHO_R32>(pl, dmat, cin, nbands, cout, s);
-        case SHO_C64:  return launch_t<SHO_C64>(pl, dmat, cin, nbands, cout, s);
+        case SHO_R64:  return launch_t<SHO_R64>(pl, dmat, cin, nbands, cout, s, shared);
+        case SHO_C128: return launch_t<SHO_C128>(pl, dmat, cin, nbands, cout, s, shared);
+        case SHO_R32:  return launch_t<SHO_R32>(pl, dmat, cin, nbands, cout, s, shared);
+        case SHO_C64:  return launch_t<SHO_C64>(pl, dmat, cin, nbands, cout, s, shared);
     }
     set_error("sho_dmul: bad dtype");
     return SHO_ERR_INVALID_ARG;

@@ -143,7 +143,8 @@ sho_status tables1d_build(const sho_plan* p, sho_tables1d** out, size_t* bytes_n
 sho_status launch_add_stored(const sho_plan* p, const sho_tables* t, const void* coeff, int nbands, void* psi, cudaStream_t s);
 sho_status launch_to_x_fastest(const sho_plan* p, const void* psi_bf, int nbands, int b0, int nb, void* psi_xf, cudaStream_t s);
 sho_status launch_from_x_fastest(const sho_plan* p, const void* psi_xf, int nbands, int b0, int nb, void* psi_bf, cudaStream_t s);
-sho_status launch_dmul(const sho_plan* p, const double* dmat, const void* cin, int nbands, void* cout, cudaStream_t s);
+// shared: dmat is ONE [N_SHO][N_SHO] matrix applied to every atom (sho_transform) instead of one per atom
+sho_status launch_dmul(const sho_plan* p, const double* dmat, const void* cin, int nbands, void* cout, cudaStream_t s, bool shared = false);
 sho_status launch_project_stored(const sho_plan* p, const sho_tables* t, const void* psi, int nbands, void* coeff,
                                  cudaStream_t s);
 sho_status tables_build(const sho_plan* p, sho_tables** out, size_t* bytes_needed, cudaStream_t s);

@@ -131,3 +131,18 @@ def test_workload_generator_is_seeded_and_shaped_like_the_configs():
     w = workloads.make(2, size="small")
     assert np.array_equal(w.psi_band(1), w.psi()[1])
     assert not np.array_equal(w.psi_band(0), w.psi_band(1))
+
+
+def test_umatrix_and_rlm_index_match_the_oracle():
+    """sho_umatrix is host code (no GPU): the library's exact quadrature against the oracle's, and the spherical
+    index map against the oracle's literal enumeration."""
+    for numax in (0, 1, 2, 4, 7, 9):
+        U = sho.umatrix(numax)
+        Uo = oracle.umatrix(numax)
+        assert U.shape == Uo.shape and np.max(np.abs(U - Uo)) < 1e-13
+        for nu in range(numax + 1):
+            for nr in range(nu // 2 + 1):
+                l = nu - 2 * nr
+                for m in range(-l, l + 1):
+                    assert sho.rlm_index(nr, l, m, numax) == oracle.rlm_index(nr, l, m, numax)
+    assert sho.rlm_index(0, 3, 0, 2) == -1 and sho.rlm_index(0, 1, 2, 3) == -1

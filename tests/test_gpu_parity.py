@@ -667,6 +667,32 @@ def test_band_fastest_layout_entry_points(sho, dtype, nb, wb):
         plan.close()
 
 
+@pytest.mark.parametrize("k,dtype", [(2, None), (5, None), (4, "r32")])
+def test_transform_to_the_spherical_representation(sho, k, dtype):
+    """sho_transform with the library's U against the oracle's U applied by the oracle's dmul (f4),
+    and back with the transpose."""
+    import torch
+    w = workloads.make(k, size="small", dtype=dtype)
+    if dtype in ("r32", "r64"):
+        w.kfrac = None
+    wide = np.complex128 if w.is_complex else np.float64
+    plan = sho.plan_for(w)
+    try:
+        c = w.coeff(plan.nsho)
+        Uo = oracle.umatrix(w.numax)
+        ref = oracle.dmul(np.tile(Uo, (w.natoms, 1, 1)), c.astype(wide))
+        U = sho.umatrix(w.numax)
+        d_c = _dev(c)
+        out = plan.transform(_dev(U), d_c)
+        back = plan.transform(_dev(np.ascontiguousarray(U.T)), out)
+        torch.cuda.synchronize()
+        tol = TOL[w.dtype]
+        assert np.abs(out.cpu().numpy().astype(wide) - ref).max() <= tol * np.abs(ref).max()
+        assert np.abs(back.cpu().numpy().astype(wide) - c.astype(wide)).max() <= (1e-12 if tol < 1e-6 else 1e-5) * np.abs(c).max()
+    finally:
+        plan.close()
+
+
 def test_wrong_arguments_raise(sho):
     import torch
     w = workloads.make(1)

@@ -595,3 +595,69 @@ def test_nonlocal_action_is_hermitian_for_symmetric_D(cplx):
     c = oracle.project(ng, h, per, kfrac, pos, sigma, numax, psi, rcut_sigma=5.0)
     ref = oracle.add(ng, h, per, kfrac, pos, sigma, numax, c, np.zeros_like(psi), rcut_sigma=5.0)
     assert np.array_equal(V(psi, one), ref)
+
+
+# ----------------------------------------------------------------------------------------------
+# f4: the unitary transform U between Cartesian and spherical states (eq. (10)-(11))
+
+
+def test_umatrix_textbook_shells(golden):
+    """s, p, d and s* rows against the values every text lists (tests/golden/umatrix_textbook.txt); everything else
+    inside the shells nu <= 2 must vanish."""
+    U = oracle.umatrix(2)
+    want = np.zeros_like(U)
+    for nr, l, m, nx, ny, nz, v in golden("umatrix_textbook.txt"):
+        want[oracle.rlm_index(int(nr), int(l), int(m), 2), oracle.index(int(nx), int(ny), int(nz), 2)] = float(v)
+    assert np.max(np.abs(U - want)) < 1e-14
+    # the same shells are the leading block of a larger basis in the spherical order, and the Cartesian columns agree
+    U5 = oracle.umatrix(5)
+    for nr, l, m, nx, ny, nz, v in golden("umatrix_textbook.txt"):
+        assert U5[oracle.rlm_index(int(nr), int(l), int(m), 5), oracle.index(int(nx), int(ny), int(nz), 5)] == pytest.approx(float(v), abs=1e-14)
+
+
+@pytest.mark.parametrize("numax", [0, 1, 3, 6])
+def test_umatrix_is_orthogonal_and_block_diagonal_in_nu(numax):
+    """Unitarity ("a unitary transform") and eq. (11): elements vanish unless l + 2 nr = nx + ny + nz."""
+    U = oracle.umatrix(numax)
+    n = oracle.nsho(numax)
+    assert U.shape == (n, n)
+    assert np.max(np.abs(U @ U.T - np.eye(n))) < 1e-13 and np.max(np.abs(U.T @ U - np.eye(n))) < 1e-13
+    nu_row = np.zeros(n, int)
+    seen = set()
+    for nu in range(numax + 1):
+        for nr in range(nu // 2 + 1):
+            l = nu - 2 * nr
+            for m in range(-l, l + 1):
+                i = oracle.rlm_index(nr, l, m, numax)
+                assert 0 <= i < n and i not in seen
+                seen.add(i)
+                nu_row[i] = nu
+    assert len(seen) == n                                                   # the spherical index is a bijection too
+    for nz in range(numax + 1):
+        for ny in range(numax + 1 - nz):
+            for nx in range(numax + 1 - nz - ny):
+                col = U[:, oracle.index(nx, ny, nz, numax)]
+                assert np.max(np.abs(col[nu_row != nx + ny + nz]), initial=0.0) < 1e-14
+
+
+def test_umatrix_rotates_a_spherically_symmetric_function_into_l0_only():
+    """A property that does not use the matrix's own construction: psi(r) = exp(-r^2 / (2 s^2)) is spherically symmetric,
+    so its Cartesian projection coefficients (closed form of pin P3, a product of 1D overlaps) must map under U onto the
+    l = 0 states only."""
+    numax, sigma, s = 6, 1.0, 0.8
+    one = [gaussian_overlap_closed(n, sigma, s, 0.0) for n in range(numax + 1)]
+    c = np.zeros(oracle.nsho(numax))
+    for nz in range(numax + 1):
+        for ny in range(numax + 1 - nz):
+            for nx in range(numax + 1 - nz - ny):
+                c[oracle.index(nx, ny, nz, numax)] = one[nx] * one[ny] * one[nz]
+    d = oracle.umatrix(numax) @ c
+    for nu in range(numax + 1):
+        for nr in range(nu // 2 + 1):
+            l = nu - 2 * nr
+            for m in range(-l, l + 1):
+                v = d[oracle.rlm_index(nr, l, m, numax)]
+                if l > 0:
+                    assert abs(v) < 1e-13
+    assert abs(d[oracle.rlm_index(0, 0, 0, numax)]) > 1.0                   # and the s states carry it
+    assert abs(np.sum(d * d) - np.sum(c * c)) < 1e-13
