@@ -227,15 +227,21 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
     }
     p->n_nonempty = (int32_t)nonempty.size();
     {   // x load steps of the project kernel per row block (one 128-byte line per row and step, real data)
-        const int cwx = (dtype == SHO_R32) ? 32 : 16;
-        int64_t steps = 0, odd = 0;
+        // steps of cwx columns (real data; complex data: half of that) from a 128-byte line or from a 32-byte lane span
+        const int cwx = (dtype == SHO_R32) ? 32 : (is_complex(dtype) ? (dtype == SHO_C64 ? 16 : 8) : 16), epl = cwx / 4;
+        int64_t steps[2] = { 0, 0 }, odd[2] = { 0, 0 };
         for (int a : nonempty) {
             const AtomDev& at = p->atoms[(size_t)a];
-            const int xs0 = floordiv_h(at.lo[0], cwx) * cwx;
-            const int ks = (at.hi[0] - xs0 + cwx) / cwx;
-            steps += ks; odd += ks & 1;
+            for (int v = 0; v < 2; ++v) {
+                const int al = v ? epl : cwx;
+                const int xs0 = floordiv_h(at.lo[0], al) * al;
+                const int ks = (at.hi[0] - xs0 + cwx) / cwx;
+                steps[v] += ks; odd[v] += ks & 1;
+            }
         }
-        p->proj_odd_steps = steps ? (double)odd / (double)steps : 0.0;
+        p->proj_xalign_span = (steps[1] * 10 < steps[0] * 9) ? 1 : 0;
+        const int v = p->proj_xalign_span;
+        p->proj_odd_steps = steps[v] ? (double)odd[v] / (double)steps[v] : 0.0;
     }
     p->order = nonempty;
     p->order.insert(p->order.end(), empty.begin(), empty.end());

@@ -78,6 +78,7 @@ struct sho_plan {
     int32_t n_nonempty;
     int32_t max_n[3];                      // largest box extent per axis
     int64_t sum_box;                       // sum over atoms of box points
+    int32_t proj_xalign_span;              // project: x steps start at a 32-byte lane span instead of a 128-byte line (saves > 10 % of them)
     double proj_odd_steps;                 // real data: share of x load steps lost if they are issued in pairs (see launch_project)
     // device mirrors
     sho::AtomDev* d_atoms;

@@ -47,6 +47,7 @@ struct ProjParams {
     int32_t cnb;               // bands per atom in the coefficient array (>= nbands: a chunk of a wider array)
     int32_t n_work_atoms;      // atoms with a non-empty box (first entries of order[])
     int32_t kx_cap, yb_cap, nz_cap;    // capacities of the shared tables: x steps, 8-row blocks, planes
+    int32_t xalign_span;       // x steps start at a lane-span boundary instead of a 128-byte line (plan statistic)
     int32_t fast;              // 32-byte loads are legal: psi 32-byte aligned and Nx a multiple of the lane span
     long long band_stride;     // elements between bands
 };
@@ -146,8 +147,12 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
     const bool fast = p.fast != 0;
 
     const int nyl = at.hi[1] - at.lo[1] + 1, nzl = at.hi[2] - at.lo[2] + 1;
-    // x: steps of CWX columns (one 128-byte line per row) starting at a line-aligned column
-    const int xs0 = floordiv(at.lo[0], CWX) * CWX;
+    // x: steps of CWX columns (128 bytes per row).  They start at a 128-byte line, or -- when the plan found that this
+    // saves more than a tenth of the steps -- at the lane-span boundary (32 bytes) at or before the box: such a step
+    // touches two lines per row but the same sectors (cfg 3: 4 steps instead of 4.75 on average, 1.90 -> 1.54 ms;
+    // cfg 4: 8 instead of 8.5, but 2 % slower: its L1 data pipe is 89 % busy, so it keeps line-aligned steps)
+    const int xalign = p.xalign_span ? EPL : CWX;
+    const int xs0 = floordiv(at.lo[0], xalign) * xalign;
     const int KX = (at.hi[0] - xs0 + CWX) / CWX;
     // y: blocks of 8 rows (the N extent of the x-stage MMA)
     const int NYB = (nyl + 7) >> 3;
@@ -593,6 +598,7 @@ static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void
     p.nbands = nbands;
     p.cnb = cnb;
     p.n_work_atoms = pl->n_nonempty;
+    p.xalign_span = pl->proj_xalign_span;
     p.kx_cap = (pl->max_n[0] + 2 * (CWX - 1)) / CWX + 2;     // + the twice-scheduled image-boundary step
     p.yb_cap = (pl->max_n[1] + 7) / 8 + 1;
     p.nz_cap = pl->max_n[2] + 1;
