@@ -199,7 +199,7 @@ sho_status sho_add_bf(const sho_plan* plan, const void* coeff, int32_t nbands, v
  * out, and synchronise the stream before returning.  They use a device workspace owned by the plan
  * (the only hot-path calls that may allocate; it is grown on demand and bounded by the chunk size, not
  * by nbands).  The bands are independent (eq. (25)), so the calls work in chunks of bands
- * (about 512 MB of psi each; environment variable SHO_HOST_CHUNK_BANDS overrides the chunk size)
+ * (about 128 MB of psi each; environment variable SHO_HOST_CHUNK_BANDS overrides the chunk size)
  * through a ring of three chunk buffers and overlap the H2D copy of the next chunk, the kernels of this
  * one and the D2H copy of the previous one on two copy streams owned by the plan; all of it is ordered
  * after the work already queued on cuda_stream.  If a step fails mid-way the call waits for everything

@@ -645,7 +645,9 @@ static sho_status ws_reserve(void** ws, size_t* have, size_t need, const char* w
     return SHO_OK;
 }
 
-// bands per chunk: about 512 MB of psi, an even number (the add kernel pairs real bands), at most 16 chunks
+// bands per chunk: about 128 MB of psi (the first upload and the last download are not overlapped with anything, so
+// small chunks win: cfg 5 end to end 177 / 165 / 160 / 158 ms with 8 / 4 / 2 / 1 bands of 113 MB per chunk), an even
+// number (the add kernel pairs real bands), at most 64 chunks
 static int host_chunk_bands(const sho_plan* plan, int nbands)
 {
     if (const char* env = std::getenv("SHO_HOST_CHUNK_BANDS")) {            // tuning / test knob
@@ -653,8 +655,8 @@ static int host_chunk_bands(const sho_plan* plan, int nbands)
         if (v > 0) return std::min(v, nbands);
     }
     const double band_bytes = (double)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * elem_size(plan->dtype);
-    int cb = (int)std::max(1.0, std::floor(512.0e6 / band_bytes));
-    cb = std::max(cb, (nbands + 15) / 16);
+    int cb = (int)std::max(1.0, std::floor(128.0e6 / band_bytes));
+    cb = std::max(cb, (nbands + 63) / 64);
     if (cb > 1) cb += cb & 1;
     return std::min(cb, nbands);
 }
