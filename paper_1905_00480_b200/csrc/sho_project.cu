@@ -28,6 +28,8 @@
 //       __syncthreads per round (double-buffered), coalesced store of N_SHO coefficients at the end.
 // Bloch phases never touch the inner loop: the x-phase is one accumulator rotation at the wrap column,
 // y-phases rotate the a3 accumulators per row, the z-phase (and the last x image) is folded into a5.
+#include <algorithm>
+
 #include "sho_device.cuh"
 
 namespace sho {
@@ -46,6 +48,7 @@ struct ProjParams {
     int32_t nbands;
     int32_t cnb;               // bands per atom in the coefficient array (>= nbands: a chunk of a wider array)
     int32_t n_work_atoms;      // atoms with a non-empty box (first entries of order[])
+    int32_t bands_per_cta;     // consecutive bands one CTA projects with the tables it sampled once
     int32_t kx_cap, yb_cap, nz_cap;    // capacities of the shared tables: x steps, 8-row blocks, planes
     int32_t xalign_span;       // x steps start at a lane-span boundary instead of a 128-byte line (plan statistic)
     int32_t fast;              // 32-byte loads are legal: psi 32-byte aligned and Nx a multiple of the lane span
@@ -107,7 +110,8 @@ __device__ __forceinline__ void ldg256(const float* p, float (&r)[8])
                  : "l"(p));
 }
 
-template <int MT, int R, int DT, int G>
+template <int MT, int R, int DT, int G, int MB>
+// MB = 1: the CTA projects several bands one after the other (the band loop below); MB = 0: one band, no loop
 // three CTAs per SM for real data (80 registers; measured faster), two for complex data (128 registers)
 __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_C64 || MT == 2) ? 2 : 3) sho_project_kernel(const ProjParams p)
 {
@@ -138,9 +142,12 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int q = lane >> 2, t = lane & 3;
 
-    // work item: band-major, atoms in the plan's spatial order (neighbouring CTAs share psi in L2)
-    const int b = blockIdx.x / p.n_work_atoms;
-    const int a = p.order[blockIdx.x - b * p.n_work_atoms];
+    // work item: (group of bands_per_cta consecutive bands, atom), band-group-major, atoms in the plan's spatial order
+    // (neighbouring CTAs share psi in L2).  The CTA samples its atom's tables once and projects the bands one by one.
+    const int bgrp = blockIdx.x / p.n_work_atoms;
+    const int a = p.order[blockIdx.x - bgrp * p.n_work_atoms];
+    const int b_first = MB ? bgrp * p.bands_per_cta : bgrp;
+    const int b_end = MB ? min(b_first + p.bands_per_cta, p.nbands) : b_first + 1;
     const AtomDev at = p.atoms[a];
     const int Nx = p.g.ng[0], Ny = p.g.ng[1], Nz = p.g.ng[2];
     const int numax = p.g.numax;
@@ -256,7 +263,6 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
     }
     __syncthreads();
 
-    const real_t* psi_b = reinterpret_cast<const real_t*>(p.psi) + (size_t)b * p.band_stride * P;
     const size_t plane = (size_t)Ny * Nx;
 
     // a5 accumulators: thread n owns coefficient(s) n, n + blockDim, ...
@@ -268,9 +274,18 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
         const uint32_t pk = (n < p.g.nsho) ? p.nxyz[n] : 0u;
         myt2[j] = t2_index<MT, R>(pk & 255, (pk >> 8) & 255);
         mynz[j] = (pk >> 16) & 255;
+    }
+    const int nrounds = (nzl + kProjWarps - 1) / kProjWarps;
+    const double h3 = p.g.h * p.g.h * p.g.h;
+
+    // The bands of the group, one after the other.  The T2 buffers and their mbarriers run on across bands: the rounds
+    // are numbered through (rbase + round), so buffer and parity continue where the band before stopped.
+  for (int b = b_first, rbase = 0; b < b_end; ++b, rbase += nrounds) {
+    const real_t* psi_b = reinterpret_cast<const real_t*>(p.psi) + (size_t)b * p.band_stride * P;
+#pragma unroll
+    for (int j = 0; j < NACC; ++j)
 #pragma unroll
         for (int pp = 0; pp < P; ++pp) acc[j][pp] = 0.0;
-    }
 
     // ---- a2 helpers: plane pointer, this lane's row pointer of a row block, one group of loads ----
     auto plane_ptr = [&](int zi) -> const real_t* {
@@ -311,7 +326,6 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
 
     // The load ring: while the G steps in cur are contracted, the next G steps are in flight; the ring
     // runs on across row-block ends (over the y stage) and plane ends (over a5 and its barrier).
-    const int nrounds = (nzl + kProjWarps - 1) / kProjWarps;
     real_t cur[G][RAW];
     const real_t* rp = psi_b;                    // row pointer of the current row block for this lane
 #pragma unroll
@@ -324,7 +338,7 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
     }
     // ---- a5: z contraction of the 8 planes of one round, thread n <- coefficient n ----
     auto a5 = [&](int rnd) {
-        const double* t2r = t2s + (size_t)(rnd & 3) * kProjWarps * P * TS;
+        const double* t2r = t2s + (size_t)((rbase + rnd) & 3) * kProjWarps * P * TS;
         const int wmax = min(kProjWarps, nzl - rnd * kProjWarps);
 #pragma unroll
         for (int j = 0; j < NACC; ++j) {
@@ -349,7 +363,7 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
 
     for (int round = 0; round < nrounds; ++round) {
         const int zi = round * kProjWarps + warp;
-        double* t2w = t2s + ((size_t)(round & 3) * kProjWarps + warp) * P * TS;
+        double* t2w = t2s + ((size_t)((rbase + round) & 3) * kProjWarps + warp) * P * TS;
         if (zi < nzl) {
             const real_t* pz = plane_ptr(zi);
             const real_t* pzn = (zi + kProjWarps < nzl) ? plane_ptr(zi + kProjWarps) : pz;
@@ -556,13 +570,12 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
         // so a warp waits for the others only when it is more than a whole plane ahead of the slowest.  Buffer
         // reuse is safe with four: a5(r-4) precedes arrive(r-2) in every warp, and this warp waited for (r-2).
         __syncwarp();
-        if (lane == 0) mbar_arrive(t2bar + (round & 3));
-        if (round >= 1) { mbar_wait(t2bar + ((round - 1) & 3), ((round - 1) >> 2) & 1); a5(round - 1); }
+        if (lane == 0) mbar_arrive(t2bar + ((rbase + round) & 3));
+        if (round >= 1) { mbar_wait(t2bar + ((rbase + round - 1) & 3), ((rbase + round - 1) >> 2) & 1); a5(round - 1); }
     }
-    if (nrounds >= 1) { mbar_wait(t2bar + ((nrounds - 1) & 3), ((nrounds - 1) >> 2) & 1); a5(nrounds - 1); }
+    if (nrounds >= 1) { mbar_wait(t2bar + ((rbase + nrounds - 1) & 3), ((rbase + nrounds - 1) >> 2) & 1); a5(nrounds - 1); }
 
     // ---- store: c[a][b][n] = h^3 * acc (reading A7) ----
-    const double h3 = p.g.h * p.g.h * p.g.h;
     real_t* cout = reinterpret_cast<real_t*>(p.coeff) + ((size_t)a * p.cnb + b) * p.g.nsho * P;
 #pragma unroll
     for (int j = 0; j < NACC; ++j) {
@@ -572,6 +585,7 @@ __global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_
             for (int pp = 0; pp < P; ++pp) cout[(size_t)n * P + pp] = (real_t)(h3 * acc[j][pp]);
         }
     }
+  }     // bands of the group
 }
 
 template <typename T>
@@ -610,11 +624,25 @@ static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void
                   pl->max_n[0], pl->max_n[1], pl->max_n[2], smem);
         return SHO_ERR_UNSUPPORTED;
     }
-    auto kern = sho_project_kernel<MT, R, DT, G>;
+    // bands per CTA: the tables of an atom (and the CTA's start-up) are paid once per CTA; with many bands and small
+    // boxes (the paper's workload: 1024 bands, 28^3 points) that is a good part of a one-band CTA's life (paper-nu5
+    // project 13.6 -> 12.1 ms).  As many bands as leave about 20 full waves of CTAs, at most 8 -- and only while the
+    // bands the resident CTAs spread over stay in L2 together (24 MB): CTAs that run at the same time read
+    // neighbouring boxes of the same band, and with 7 bands of 113 MB per CTA cfg 5 takes 49.9 instead of 38.3 ms.
+    int nsm = 0;
+    cudaError_t e0 = cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, pl->device);
+    if (e0 != cudaSuccess) return cuda_fail(e0, "cudaDeviceGetAttribute(project)");
+    const long long per_wave = (long long)std::max(nsm, 1) * ((CPLX || MT == 2) ? 2 : 3);
+    const double band_bytes = (double)pl->g.ng[0] * pl->g.ng[1] * pl->g.ng[2] * elem_size(pl->dtype);
+    const long long by_l2 = std::max<long long>(1, (long long)(24.0e6 / band_bytes));
+    const int bpc = (int)std::min<long long>(std::min<long long>(8, by_l2),
+                                             std::max<long long>(1, (long long)pl->n_nonempty * nbands / (20 * per_wave)));
+    p.bands_per_cta = bpc;
+    const long long nblocks = (long long)pl->n_nonempty * ((nbands + bpc - 1) / bpc);
+    if (nblocks > 0x7fffffffLL) { set_error("sho_project: natoms*nbands too large"); return SHO_ERR_UNSUPPORTED; }
+    auto kern = (bpc > 1) ? sho_project_kernel<MT, R, DT, G, 1> : sho_project_kernel<MT, R, DT, G, 0>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(project)");
-    const long long nblocks = (long long)pl->n_nonempty * nbands;
-    if (nblocks > 0x7fffffffLL) { set_error("sho_project: natoms*nbands too large"); return SHO_ERR_UNSUPPORTED; }
     if (nblocks > 0) {
         kern<<<(unsigned)nblocks, kProjWarps * 32, smem, s>>>(p);
         e = cudaGetLastError();
