@@ -29,6 +29,7 @@
 // Bloch phases never touch the inner loop: the x-phase is one accumulator rotation at the wrap column,
 // y-phases rotate the a3 accumulators per row, the z-phase (and the last x image) is folded into a5.
 #include <algorithm>
+#include <cstdlib>
 
 #include "sho_device.cuh"
 
@@ -635,8 +636,12 @@ static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void
     const long long per_wave = (long long)std::max(nsm, 1) * ((CPLX || MT == 2) ? 2 : 3);
     const double band_bytes = (double)pl->g.ng[0] * pl->g.ng[1] * pl->g.ng[2] * elem_size(pl->dtype);
     const long long by_l2 = std::max<long long>(1, (long long)(24.0e6 / band_bytes));
-    const int bpc = (int)std::min<long long>(std::min<long long>(8, by_l2),
+    int bpc = (int)std::min<long long>(std::min<long long>(8, by_l2),
                                              std::max<long long>(1, (long long)pl->n_nonempty * nbands / (20 * per_wave)));
+    if (const char* env = std::getenv("SHO_PROJECT_BANDS_PER_CTA")) {      // test knob: the band loop on small inputs
+        const int v = std::atoi(env);
+        if (v >= 1) bpc = std::min(v, std::max(nbands, 1));
+    }
     p.bands_per_cta = bpc;
     const long long nblocks = (long long)pl->n_nonempty * ((nbands + bpc - 1) / bpc);
     if (nblocks > 0x7fffffffLL) { set_error("sho_project: natoms*nbands too large"); return SHO_ERR_UNSUPPORTED; }

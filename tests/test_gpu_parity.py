@@ -275,7 +275,19 @@ def _sample_bands(nb, n=8):
     return sorted(set([0, 1, nb // 3, nb // 2 - 1, nb // 2, (2 * nb) // 3 + 1, nb - 2, nb - 1][:n]) & set(range(nb)))
 
 
-@pytest.mark.parametrize("k,dtype", [(3, None), (4, None), (4, "r32"), (5, None)])
+@pytest.mark.parametrize("bpc", [2, 3, 8])
+def test_project_band_loop_of_a_cta(sho, bpc, monkeypatch):
+    """A CTA of sho_project may project several consecutive bands with the tables it sampled once (the launch picks
+    that for many bands of a small grid: the paper's workload).  Forced here on small inputs through the library's
+    test knob: band counts that are and are not multiples of the group, real and complex data, remainder rows."""
+    monkeypatch.setenv("SHO_PROJECT_BANDS_PER_CTA", str(bpc))
+    for w in (workloads.make_paper(5, "r64", size="small"), workloads.make(5, size="small"), workloads.make(2, size="small")):
+        for nb in (w.nbands, 5):
+            w.nbands = nb
+            run_case(sho, w, stored=False)
+
+
+@pytest.mark.parametrize("k,dtype", [(3, None), (4, None), (4, "r32"), (5, None), ("paper", "r64")])
 def test_full_size_config_sampled(sho, k, dtype):
     """BASELINE.json config k at its full size, in the launch configuration bench.py times (all bands, device
     inputs from a seeded torch generator), sampled as SURVEY 8(d) asks:
@@ -286,7 +298,7 @@ def test_full_size_config_sampled(sho, k, dtype):
                middle plane) for 8 bands, plus 4096 random points for ALL bands, every value computed
                point-wise by the oracle.  Norms of reading A13 over the samples."""
     import torch
-    w = workloads.make(k, dtype=dtype)
+    w = workloads.make_paper(5, dtype) if k == "paper" else workloads.make(k, dtype=dtype)   # paper: 8 bands per CTA
     if dtype in ("r32", "r64"):
         w.kfrac = None
     tol = TOL[w.dtype]
