@@ -102,6 +102,9 @@ sho_status sho_plan_info(const sho_plan* plan, int64_t info[8]);
 /*
  * Projection, on-the-fly SHO.  psi DEVICE [nbands][Nz][Ny][Nx]; coeff DEVICE [natoms][nbands][N_SHO]
  * (overwritten; atoms with an empty box get zeros).  cuda_stream is a cudaStream_t (NULL = default).
+ * Deterministic (fixed summation order, no atomics).  One CTA projects one atom and 1..8 consecutive bands
+ * (chosen per launch from the band count and the grid size; the environment variable
+ * SHO_PROJECT_BANDS_PER_CTA overrides it -- a test knob, the result does not depend on it).
  */
 sho_status sho_project(const sho_plan* plan, const void* psi, int32_t nbands, void* coeff, void* cuda_stream);
 

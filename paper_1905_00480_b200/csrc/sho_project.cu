@@ -113,8 +113,9 @@ __device__ __forceinline__ void ldg256(const float* p, float (&r)[8])
 
 template <int MT, int R, int DT, int G, int MB>
 // MB = 1: the CTA projects several bands one after the other (the band loop below); MB = 0: one band, no loop
-// three CTAs per SM for real data (80 registers; measured faster), two for complex data (128 registers)
-__global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_C64 || MT == 2) ? 2 : 3) sho_project_kernel(const ProjParams p)
+// three CTAs per SM for real data without remainder rows (80 registers; measured faster), two for complex data and for
+// real data with remainder rows (at 80 registers those spill: numax 9 on cfg 4's geometry 40.1 ms against 37.4 with two CTAs)
+__global__ void __launch_bounds__(kProjWarps * 32, (DT == SHO_C128 || DT == SHO_C64 || MT == 2 || R > 0) ? 2 : 3) sho_project_kernel(const ProjParams p)
 {
     using E = Elem<DT>;
     using S = ProjSmem<MT, R, DT>;
@@ -633,7 +634,7 @@ static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void
     int nsm = 0;
     cudaError_t e0 = cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, pl->device);
     if (e0 != cudaSuccess) return cuda_fail(e0, "cudaDeviceGetAttribute(project)");
-    const long long per_wave = (long long)std::max(nsm, 1) * ((CPLX || MT == 2) ? 2 : 3);
+    const long long per_wave = (long long)std::max(nsm, 1) * ((CPLX || MT == 2 || R > 0) ? 2 : 3);
     const double band_bytes = (double)pl->g.ng[0] * pl->g.ng[1] * pl->g.ng[2] * elem_size(pl->dtype);
     const long long by_l2 = std::max<long long>(1, (long long)(24.0e6 / band_bytes));
     int bpc = (int)std::min<long long>(std::min<long long>(8, by_l2),

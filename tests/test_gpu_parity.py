@@ -285,6 +285,19 @@ def test_project_band_loop_of_a_cta(sho, bpc, monkeypatch):
         for nb in (w.nbands, 5):
             w.nbands = nb
             run_case(sho, w, stored=False)
+    # the grouping changes which CTA computes a band, not how: bit-identical coefficients
+    import torch
+    w = workloads.make(5, size="small")
+    plan = sho.plan_for(w)
+    try:
+        psi = _dev(w.psi())
+        c_grouped = plan.project(psi).clone()
+        monkeypatch.setenv("SHO_PROJECT_BANDS_PER_CTA", "1")
+        c_single = plan.project(psi)
+        torch.cuda.synchronize()
+        assert torch.equal(torch.view_as_real(c_grouped), torch.view_as_real(c_single))
+    finally:
+        plan.close()
 
 
 @pytest.mark.parametrize("k,dtype", [(3, None), (4, None), (4, "r32"), (5, None), ("paper", "r64")])
