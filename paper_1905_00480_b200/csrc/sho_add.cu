@@ -172,7 +172,13 @@ __device__ __forceinline__ void add_zpair(const real_t* __restrict__ a0p, const 
     }
 }
 
-template <int KQ, int DT>
+// MIX (numax = 8, 9 only): the third K step of the y stage holds just ny = 8, 9, and the x stage spends one MMA per
+// channel on the three pairs (ny, nx) = (8,0), (8,1), (9,0) and another on (0,8), (0,9), (1,8).  With MIX the free
+// half of that y K step carries ny = 0, 1 a second time -- A fragment (phi_8, phi_9, phi_0, phi_1)(y) -- against the
+// partial x sums over nx = 8, 9 only, and ONE x-stage MMA with the A fragment (phi_0, phi_1, phi_8, phi_9)(x) yields
+// its four B columns: T1[x][8], T1[x][9] (from nx = 0, 1) and the nx = 8, 9 parts of T1[x][0], T1[x][1].  Three
+// x-stage MMAs per plane and channel instead of four, two shared-memory loads fewer; nothing else changes.
+template <int KQ, int DT, int MIX>
 __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel(const __grid_constant__ AddParams p)
 {
     using E = Elem<DT>;
@@ -186,6 +192,7 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
     constexpr int FXYS = S::FXYS, FZS = S::FZS;
     constexpr int MTC = (KQ <= 2) ? 4 : 3;     // z-stage row tiles whose coefficients a producer lane holds at once
     static_assert(kAddTX == 8 && kAddTZ == 8, "one 8x8 MMA block per x / z extent");
+    static_assert(!MIX || KQ == 3, "MIX is the numax = 8, 9 variant");
     constexpr int kAddXYWarps = add_xy_warps(CPLX), kAddThreads = add_threads(CPLX);
 
     extern __shared__ __align__(16) double smem[];
@@ -258,6 +265,10 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
         for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
             for (int ks = 0; ks < KQ; ++ks) t2off[nt][ks] = p.t2pos[16 * (8 * nt + 4 * (q & 1) + (q >> 1)) + 4 * ks + t];
+        // MIX: B fragment of the one mixed x-stage MMA, B[k = t][column q]: columns 0, 2 <- (8, nx = t), (9, nx = t) for t < 2;
+        // columns 4, 6 <- (0, nx = 6 + t), (1, nx = 6 + t) for t >= 2; everything else reads the zero column
+        const int t2off_mix = !MIX ? 0 : (int)p.t2pos[(q == 0 && t < 2) ? 16 * 8 + t : (q == 2 && t < 2) ? 16 * 9 + t :
+                                                       (q == 4 && t >= 2) ? 6 + t : (q == 6 && t >= 2) ? 16 + 6 + t : 255];
 
         int slot = 0, ph = 0;
         const double* fxy = FXY + lane;
@@ -299,10 +310,11 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
                     for (int ks = 0; ks < KQ; ++ks)
 #pragma unroll
                         for (int nt = 0; nt < NT; ++nt)
-                            if (8 * nt + 4 * ks <= 4 * KQ - 4) {            // the block holds some ny+nx <= numax (numax >= 4 KQ - 4)
+                            if (MIX ? (nt == 0 && ks < 2) || (nt == 1 && ks == 2) : 8 * nt + 4 * ks <= 4 * KQ - 4) {   // the block holds some ny+nx <= numax (numax >= 4 KQ - 4)
                                 const double a = fxy[(8 * KQ + ks) * 32];
-                                dmma(D1[nt][0][0], D1[nt][0][1], a, t2p[t2off[nt][ks]]);
-                                dmma(D1[nt][1][0], D1[nt][1][1], a, t2p[(size_t)kAddTZ * npp + t2off[nt][ks]]);
+                                const int o = (MIX && nt == 1) ? t2off_mix : t2off[nt][ks];
+                                dmma(D1[nt][0][0], D1[nt][0][1], a, t2p[o]);
+                                dmma(D1[nt][1][0], D1[nt][1][1], a, t2p[(size_t)kAddTZ * npp + o]);
                             }
                     // A predicated-off DMMA still takes its 16 cycles of the pipe (measured), and the compiler
                     // predicates a short "if": enter the unrolled blocks by a jump and leave them by a branch instead.
@@ -388,6 +400,10 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
         for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
             for (int ks = 0; ks < KQ; ++ks) t2off[nt][ks] = p.t2pos[16 * (8 * nt + 4 * (q & 1) + (q >> 1)) + 4 * ks + t];
+        // MIX: B fragment of the one mixed x-stage MMA, B[k = t][column q]: columns 0, 2 <- (8, nx = t), (9, nx = t) for t < 2;
+        // columns 4, 6 <- (0, nx = 6 + t), (1, nx = 6 + t) for t >= 2; everything else reads the zero column
+        const int t2off_mix = !MIX ? 0 : (int)p.t2pos[(q == 0 && t < 2) ? 16 * 8 + t : (q == 2 && t < 2) ? 16 * 9 + t :
+                                                       (q == 4 && t >= 2) ? 6 + t : (q == 6 && t >= 2) ? 16 + 6 + t : 255];
 
         int slot = 0, ph = 0;
         const double* fxy = FXY + lane;
@@ -428,8 +444,8 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
                     for (int ks = 0; ks < KQ; ++ks)
 #pragma unroll
                         for (int nt = 0; nt < NT; ++nt)
-                            if (8 * nt + 4 * ks <= 4 * KQ - 4)              // the block holds some ny+nx <= numax (numax >= 4 KQ - 4)
-                                dmma(D1[nt][0], D1[nt][1], fxy[(8 * KQ + ks) * 32], t2p[t2off[nt][ks]]);
+                            if (MIX ? (nt == 0 && ks < 2) || (nt == 1 && ks == 2) : 8 * nt + 4 * ks <= 4 * KQ - 4)   // the block holds some ny+nx <= numax
+                                dmma(D1[nt][0], D1[nt][1], fxy[(8 * KQ + ks) * 32], t2p[(MIX && nt == 1) ? t2off_mix : t2off[nt][ks]]);
                     // The touched 8-row blocks are ytlo..ythi.  A predicated-off DMMA still takes its 16 cycles of
                     // the pipe (measured), and the compiler predicates a short "if": enter the unrolled blocks by
                     // a jump and leave them by a branch instead.
@@ -582,6 +598,8 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
                     for (int kk = 0; kk < KQ; ++kk) {
                         double2 a, c;
                         a.x = v[4 * kk]; a.y = v[4 * kk + 1]; c.x = v[4 * kk + 2]; c.y = v[4 * kk + 3];
+                        if (MIX && kk == 2 && d == 1) { c.x = v[0]; c.y = v[1]; }                     // y: (phi_8, phi_9, phi_0, phi_1)
+                        if (MIX && kk == 2 && d == 0) { c = a; a.x = v[0]; a.y = v[1]; }              // x: (phi_0, phi_1, phi_8, phi_9)
                         *reinterpret_cast<double2*>(dst + kk * 32) = a;
                         *reinterpret_cast<double2*>(dst + kk * 32 + 2) = c;
                     }
@@ -638,7 +656,7 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
     }
 }
 
-template <int KQ, int DT>
+template <int KQ, int DT, int MIX>
 static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb, const sho_tables1d* t1)
 {
     using S = AddSmem<KQ>;
@@ -678,7 +696,7 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
         set_error("sho_add: numax = %d needs %zu bytes of shared memory (> 227 KB)", pl->g.numax, smem);
         return SHO_ERR_UNSUPPORTED;
     }
-    auto kern = sho_add_kernel<KQ, DT>;
+    auto kern = sho_add_kernel<KQ, DT, MIX>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(add)");
     const int nchunk = CPLX ? nbands : (nbands + 1) / 2;
@@ -699,10 +717,11 @@ template <int DT>
 static sho_status launch_kq(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb, const sho_tables1d* t1)
 {
     switch ((pl->g.numax + 4) >> 2) {          // K steps of four n values that hold n <= numax
-        case 1: return launch_t<1, DT>(pl, coeff, nbands, psi, s, cnb, t1);
-        case 2: return launch_t<2, DT>(pl, coeff, nbands, psi, s, cnb, t1);
-        case 3: return launch_t<3, DT>(pl, coeff, nbands, psi, s, cnb, t1);
-        default: return launch_t<4, DT>(pl, coeff, nbands, psi, s, cnb, t1);
+        case 1: return launch_t<1, DT, 0>(pl, coeff, nbands, psi, s, cnb, t1);
+        case 2: return launch_t<2, DT, 0>(pl, coeff, nbands, psi, s, cnb, t1);
+        case 3: return pl->g.numax <= 9 ? launch_t<3, DT, 1>(pl, coeff, nbands, psi, s, cnb, t1)
+                                        : launch_t<3, DT, 0>(pl, coeff, nbands, psi, s, cnb, t1);
+        default: return launch_t<4, DT, 0>(pl, coeff, nbands, psi, s, cnb, t1);
     }
 }
 
