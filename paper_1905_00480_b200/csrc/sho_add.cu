@@ -110,7 +110,8 @@ __device__ __forceinline__ double exp_neg(double x, const double* __restrict__ t
 
 // H_n(xi) exp(-xi^2/2) (sqrt(pi) sigma)^(-1/2) scale[n], n < NV, by the paper's monic recurrence (eq. (31),
 // PAPER.md:283-284) carried on p_n = H_n g; scale[n] = sqrt(2^n/n!) makes the functions orthonormal (reading A1)
-template <int NV>
+// NC <= NV functions are computed, the rest are zeros (NC = 10 when numax <= 9 is known at compile time)
+template <int NV, int NC>
 __device__ __forceinline__ void hermite_gauss_s(double u, double inv_sigma, double pref, const double* __restrict__ scale,
                                                 const double* __restrict__ exptab, double (&out)[NV])
 {
@@ -118,10 +119,13 @@ __device__ __forceinline__ void hermite_gauss_s(double u, double inv_sigma, doub
     double pm = 0.0, pc = exp_neg(-0.5 * xi * xi, exptab) * pref;
 #pragma unroll
     for (int n = 0; n < NV; ++n) {
+        if (n >= NC) { out[n] = 0.0; continue; }
         out[n] = pc * scale[n];
-        const double pn = xi * pc - (0.5 * (double)n) * pm;
-        pm = pc;
-        pc = pn;
+        if (n + 1 < NC) {
+            const double pn = xi * pc - (0.5 * (double)n) * pm;
+            pm = pc;
+            pc = pn;
+        }
     }
 }
 
@@ -587,7 +591,7 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
                     if (valid && p.tab1d) {
                         stored1d_lookup<NV>(p.tab1d, p.tab1d_off[en->atom], en->lo, en->hi, d, iu, p.g.numax, true, v);
                     } else if (valid) {
-                        hermite_gauss_s<NV>(displacement(iu, p.g.h, en->pos[d]), inv_sigma, pref, p.hz, EXPT, v);
+                        hermite_gauss_s<NV, (MIX ? 10 : NV)>(displacement(iu, p.g.h, en->pos[d]), inv_sigma, pref, p.hz, EXPT, v);
                     } else {
 #pragma unroll
                         for (int n = 0; n < NV; ++n) v[n] = 0.0;
