@@ -383,6 +383,30 @@ def test_full_size_config_sampled(sho, k, dtype):
         plan.close()
 
 
+@pytest.mark.parametrize("case", range(24))
+def test_seeded_random_geometries(sho, case):
+    """Seeded random small problems, every one compared with the oracle in full (project, add, stored variants): odd
+    grid dims, any mix of periodic and isolated axes, atoms inside, on the faces and well outside the cell, sigma such
+    that a box is at most as wide as the cell, numax 0 .. 11 (every K-step count, the remainder rows of numax 8, 9 and
+    their shared K step in the add), 1 .. 5 bands, all four element types, random Bloch phases for complex data."""
+    rng = np.random.default_rng(20260000 + case)
+    ng = tuple(int(v) for v in rng.integers(9, 41, 3))
+    periodic = tuple(int(v) for v in rng.integers(0, 2, 3))
+    h = float(rng.choice([0.2, 0.25, 0.3]))
+    numax = int(rng.integers(0, 12)) if case % 3 else int(rng.choice([8, 9]))
+    dtype = ["r64", "c128", "r32", "c64"][case % 4]
+    natoms = int(rng.integers(1, 6))
+    L = np.array(ng) * h
+    pos = (rng.random((natoms, 3)) * 2.0 - 0.5) * L                    # from half a cell before to half a cell behind
+    smax = 0.999 * (min(ng) - 1) * h / 12.0                            # 6 sigma on both sides fit the narrowest axis
+    sigma = rng.uniform(0.45 * smax, smax, natoms)
+    kfrac = None
+    if dtype in ("c128", "c64"):
+        kfrac = tuple(float(k) if per else 0.0 for k, per in zip(rng.uniform(-0.5, 0.5, 3), periodic))
+    w = _custom(ng, periodic, pos, sigma, numax, int(rng.integers(1, 6)), dtype=dtype, h=h, kfrac=kfrac, seed=500 + case)
+    run_case(sho, w, stored=(case % 2 == 0))
+
+
 def test_box_exactly_as_wide_as_the_cell(sho):
     # periodic box of exactly N points on x (every grid point once, one wrap)
     ng = (24, 40, 40)
