@@ -69,10 +69,10 @@ template <int KQ>
 struct AddSmem {
     static constexpr int FXYS = 9 * KQ * 32;
     static constexpr int FZS = KQ * 32;
-    static __host__ __device__ int t2s(int npp) { return 2 * kAddTZ * npp; }
+    static __host__ __device__ constexpr int t2s(int npp) { return 2 * kAddTZ * npp; }
     // z-stage A fragments of one pair in the element type of the data: [K block][lane][channel]
-    static __host__ __device__ int stg(int nblk, int real_bytes) { return ((64 * nblk * real_bytes + 15) / 16) * 2; }
-    static __host__ __device__ size_t bytes(int rd, int npw, int nmt, int nblk, int real_bytes, bool cplx)
+    static __host__ __device__ constexpr int stg(int nblk, int real_bytes) { return ((64 * nblk * real_bytes + 15) / 16) * 2; }
+    static __host__ __device__ constexpr size_t bytes(int rd, int npw, int nmt, int nblk, int real_bytes, bool cplx)
     {
         const int npp = 8 * nmt + 2;
         size_t b = 8 * ((size_t)rd * (FXYS + t2s(npp)) + (size_t)npw * (FZS + stg(nblk, real_bytes)) + 64);
@@ -81,7 +81,37 @@ struct AddSmem {
         b = (b + 7) & ~(size_t)7;
         return b + (size_t)2 * rd * 8 + 16;
     }
+    // producer warps and ring depth: every producer warp fills a slot of its own while the XY warps drain others, so
+    // rd > npw; as many of both as fit in the shared memory of one CTA per SM
+    static constexpr size_t kBudget = 224 * 1024;
+    static __host__ __device__ constexpr int pick_npw(int nmt, int nblk, int real_bytes, bool cplx)
+    {
+        int npw = kAddPWarps;
+        while (npw > 1 && bytes(npw + 2, npw, nmt, nblk, real_bytes, cplx) > kBudget) --npw;
+        return npw;
+    }
+    static __host__ __device__ constexpr int pick_rd(int npw, int nmt, int nblk, int real_bytes, bool cplx)
+    {
+        int rd = npw + 2;
+        while (rd < 2 * npw + 2 && bytes(rd + 1, npw, nmt, nblk, real_bytes, cplx) <= kBudget) ++rd;
+        return rd;
+    }
 };
+
+// Row tiles and K blocks of the z stage for a given numax, as sho_plan_create lays them out (AddZTiles): known at compile
+// time in the kernel variants that are instantiated for one numax (template parameter NX), where they turn ring depth,
+// table strides and loop bounds into constants -- the XY warps otherwise re-load them from the parameter bank per pair
+__host__ __device__ constexpr int add_nmt(int numax) { return ((numax + 1) * (numax + 2) / 2 + 7) / 8; }
+__host__ __device__ constexpr int add_nblk(int numax)
+{
+    int blk = 0;
+    for (int mt = 0; mt < add_nmt(numax); ++mt) {
+        int sm = 0;
+        while ((sm + 1) * (sm + 2) / 2 <= 8 * mt) ++sm;
+        blk += (numax - sm) / 4 + 1;
+    }
+    return blk;
+}
 
 // exp(x), x <= 0, in 11 FP64-pipe instructions (the library routine takes about 28; the producer warps share the
 // FP64 pipe with the DMMAs of the XY warps, so every instruction there waits its turn):
@@ -182,7 +212,8 @@ __device__ __forceinline__ void add_zpair(const real_t* __restrict__ a0p, const 
 // partial x sums over nx = 8, 9 only, and ONE x-stage MMA with the A fragment (phi_0, phi_1, phi_8, phi_9)(x) yields
 // its four B columns: T1[x][8], T1[x][9] (from nx = 0, 1) and the nx = 8, 9 parts of T1[x][0], T1[x][1].  Three
 // x-stage MMAs per plane and channel instead of four, two shared-memory loads fewer; nothing else changes.
-template <int KQ, int DT, int MIX>
+// NX: the numax this variant is compiled for (8, 9), or -1: any numax with this KQ, sizes at run time
+template <int KQ, int DT, int NX>
 __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel(const __grid_constant__ AddParams p)
 {
     using E = Elem<DT>;
@@ -196,19 +227,26 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
     constexpr int FXYS = S::FXYS, FZS = S::FZS;
     constexpr int MTC = (KQ <= 2) ? 4 : 3;     // z-stage row tiles whose coefficients a producer lane holds at once
     static_assert(kAddTX == 8 && kAddTZ == 8, "one 8x8 MMA block per x / z extent");
-    static_assert(!MIX || KQ == 3, "MIX is the numax = 8, 9 variant");
+    constexpr bool MIX = (NX == 8 || NX == 9);
+    constexpr bool EX = NX >= 0;
+    static_assert(!EX || ((NX + 4) >> 2) == KQ, "NX and KQ disagree");
+    constexpr int C_NMT = EX ? add_nmt(EX ? NX : 0) : 0, C_NBLK = EX ? add_nblk(EX ? NX : 0) : 0;
+    constexpr int C_RB = (int)sizeof(real_t);
+    constexpr int C_NPW = EX ? S::pick_npw(C_NMT, C_NBLK, C_RB, CPLX) : 0;
+    constexpr int C_RD = EX ? S::pick_rd(EX ? C_NPW : 1, C_NMT, C_NBLK, C_RB, CPLX) : 0;
     constexpr int kAddXYWarps = add_xy_warps(CPLX), kAddThreads = add_threads(CPLX);
 
     extern __shared__ __align__(16) double smem[];
     const int nsho = p.g.nsho;
-    const int RD = p.rd;
-    const int npp = p.npp;
-    const int nmt = p.zt.nmt;
+    const int RD = EX ? C_RD : p.rd;
+    const int npp = EX ? 8 * C_NMT + 2 : p.npp;
+    const int nmt = EX ? C_NMT : p.zt.nmt;
+    const int nblk = EX ? C_NBLK : p.nblk;
     const int T2S = S::t2s(npp);
     double* FXY = smem;                                   // [RD][9 KQ][32]     y blocks 0..7, x block 8
     double* T2 = FXY + (size_t)RD * FXYS;                 // [RD][2][8][npp]
-    const int NPW = p.npw;
-    const int STGS = S::stg(p.nblk, (int)sizeof(real_t));
+    const int NPW = EX ? C_NPW : p.npw;
+    const int STGS = S::stg(nblk, (int)sizeof(real_t));
     double* FZ = T2 + (size_t)RD * T2S;                   // [npw][KQ][32]
     double* STG = FZ + (size_t)NPW * FZS;                 // [npw][STGS]   z-stage A fragments of the pair in production, element type of the data
     double* EXPT = STG + (size_t)NPW * STGS;              // [64]  2^(j/64), see exp_neg
@@ -216,7 +254,7 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
     int32_t* META = reinterpret_cast<int32_t*>(ENTW + 2 * NPW);                  // [RD] zmask | ytlo << 8 | ythi << 16
     uint16_t* ZPOS = reinterpret_cast<uint16_t*>(META + RD);                     // [8 nmt] T2 column of z-stage row
     uint16_t* CIDX = ZPOS + 8 * nmt;                                             // [nblk][32] coefficient of an A-fragment element
-    uint64_t* full = reinterpret_cast<uint64_t*>((reinterpret_cast<uintptr_t>(CIDX + 32 * p.nblk) + 7) & ~(uintptr_t)7);   // [RD] 1 producer warp
+    uint64_t* full = reinterpret_cast<uint64_t*>((reinterpret_cast<uintptr_t>(CIDX + 32 * nblk) + 7) & ~(uintptr_t)7);   // [RD] 1 producer warp
     uint64_t* empty = full + RD;                                                 // [RD] 16 XY warps
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -246,7 +284,7 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
     // zero T2 once: its zero column stays zero (z-stage rows past the last pair write zeros there)
     for (int i = tid; i < RD * T2S; i += kAddThreads) T2[i] = 0.0;
     for (int i = tid; i < 8 * nmt; i += kAddThreads) ZPOS[i] = p.t2pos[256 + i];
-    for (int i = tid; i < 32 * p.nblk; i += kAddThreads) CIDX[i] = p.cidx[i];
+    for (int i = tid; i < 32 * nblk; i += kAddThreads) CIDX[i] = p.cidx[i];
     if (tid < 64) EXPT[tid] = exp2((double)tid * (1.0 / 64.0));
     if (tid == 0) {
         for (int i = 0; i < RD; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, kAddXYWarps); }
@@ -554,7 +592,7 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
             // fragment element: the lane copies its own (cp.async gather, zero fill for the padding elements) ----
             {
                 const real_t* c = cbase + (size_t)en->atom * catom;
-                for (int blk = 0; blk < p.nblk; ++blk) {
+                for (int blk = 0; blk < nblk; ++blk) {
                     const int n = CIDX[blk * 32 + lane];
                     const bool has = n != 0xffff;
                     const real_t* src = c + (has ? (size_t)n * P : 0);
@@ -591,7 +629,7 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
                     if (valid && p.tab1d) {
                         stored1d_lookup<NV>(p.tab1d, p.tab1d_off[en->atom], en->lo, en->hi, d, iu, p.g.numax, true, v);
                     } else if (valid) {
-                        hermite_gauss_s<NV, (MIX ? 10 : NV)>(displacement(iu, p.g.h, en->pos[d]), inv_sigma, pref, p.hz, EXPT, v);
+                        hermite_gauss_s<NV, (EX ? NX + 1 : NV)>(displacement(iu, p.g.h, en->pos[d]), inv_sigma, pref, p.hz, EXPT, v);
                     } else {
 #pragma unroll
                         for (int n = 0; n < NV; ++n) v[n] = 0.0;
@@ -660,7 +698,7 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
     }
 }
 
-template <int KQ, int DT, int MIX>
+template <int KQ, int DT, int NX>
 static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb, const sho_tables1d* t1)
 {
     using S = AddSmem<KQ>;
@@ -689,18 +727,19 @@ static sho_status launch_t(const sho_plan* pl, const void* coeff, int nbands, vo
     // others, so rd > npw; as many of both as fit in the shared memory of one CTA per SM
     p.nblk = zt.nblk;
     const int rb = (int)(esz / (CPLX ? 2 : 1));
-    const size_t budget = 224 * 1024;
-    int npw = kAddPWarps;
-    while (npw > 1 && S::bytes(npw + 2, npw, zt.nmt, zt.nblk, rb, CPLX) > budget) --npw;
-    int rd = npw + 2;
-    while (rd < 2 * npw + 2 && S::bytes(rd + 1, npw, zt.nmt, zt.nblk, rb, CPLX) <= budget) ++rd;
+    const int npw = S::pick_npw(zt.nmt, zt.nblk, rb, CPLX);
+    const int rd = S::pick_rd(npw, zt.nmt, zt.nblk, rb, CPLX);
     p.npw = npw; p.rd = rd;
+    if (NX >= 0 && (zt.nmt != add_nmt(NX >= 0 ? NX : 0) || zt.nblk != add_nblk(NX >= 0 ? NX : 0) || pl->g.numax != NX)) {
+        set_error("sho_add: internal: the plan's z-stage layout differs from the compiled one for numax = %d", NX);
+        return SHO_ERR_UNSUPPORTED;
+    }
     const size_t smem = S::bytes(rd, npw, zt.nmt, zt.nblk, rb, CPLX);
     if (smem > 227 * 1024) {
         set_error("sho_add: numax = %d needs %zu bytes of shared memory (> 227 KB)", pl->g.numax, smem);
         return SHO_ERR_UNSUPPORTED;
     }
-    auto kern = sho_add_kernel<KQ, DT, MIX>;
+    auto kern = sho_add_kernel<KQ, DT, NX>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(add)");
     const int nchunk = CPLX ? nbands : (nbands + 1) / 2;
@@ -721,11 +760,12 @@ template <int DT>
 static sho_status launch_kq(const sho_plan* pl, const void* coeff, int nbands, void* psi, cudaStream_t s, int cnb, const sho_tables1d* t1)
 {
     switch ((pl->g.numax + 4) >> 2) {          // K steps of four n values that hold n <= numax
-        case 1: return launch_t<1, DT, 0>(pl, coeff, nbands, psi, s, cnb, t1);
-        case 2: return launch_t<2, DT, 0>(pl, coeff, nbands, psi, s, cnb, t1);
-        case 3: return pl->g.numax <= 9 ? launch_t<3, DT, 1>(pl, coeff, nbands, psi, s, cnb, t1)
-                                        : launch_t<3, DT, 0>(pl, coeff, nbands, psi, s, cnb, t1);
-        default: return launch_t<4, DT, 0>(pl, coeff, nbands, psi, s, cnb, t1);
+        case 1: return launch_t<1, DT, -1>(pl, coeff, nbands, psi, s, cnb, t1);
+        case 2: return launch_t<2, DT, -1>(pl, coeff, nbands, psi, s, cnb, t1);      // NX = 5, 7 measured: 1 % slower
+        case 3: return pl->g.numax == 9 ? launch_t<3, DT, 9>(pl, coeff, nbands, psi, s, cnb, t1)
+                     : pl->g.numax == 8 ? launch_t<3, DT, 8>(pl, coeff, nbands, psi, s, cnb, t1)
+                                        : launch_t<3, DT, -1>(pl, coeff, nbands, psi, s, cnb, t1);
+        default: return launch_t<4, DT, -1>(pl, coeff, nbands, psi, s, cnb, t1);
     }
 }
 
