@@ -102,6 +102,12 @@ struct AddSmem {
 // time in the kernel variants that are instantiated for one numax (template parameter NX), where they turn ring depth,
 // table strides and loop bounds into constants -- the XY warps otherwise re-load them from the parameter bank per pair
 __host__ __device__ constexpr int add_nmt(int numax) { return ((numax + 1) * (numax + 2) / 2 + 7) / 8; }
+__host__ __device__ constexpr int add_nks(int numax, int mt)       // K steps of row tile mt: nz <= numax - s_min(mt)
+{
+    int sm = 0;
+    while ((sm + 1) * (sm + 2) / 2 <= 8 * mt) ++sm;
+    return (numax - sm) / 4 + 1;
+}
 __host__ __device__ constexpr int add_nblk(int numax)
 {
     int blk = 0;
@@ -206,13 +212,39 @@ __device__ __forceinline__ void add_zpair(const real_t* __restrict__ a0p, const 
     }
 }
 
+// The whole z stage of a pair for a numax known at compile time: row tiles MT0, MT0 + 1, ... two at a time, their K-step
+// counts and K-block offsets constants, no jump table
+template <int NX, int MT0, int BLK, bool CPLX, typename real_t>
+__device__ __forceinline__ void add_ztiles(const real_t* __restrict__ stg_lane, const double* __restrict__ fzl, bool phased,
+                                           double wr, double wi, double* __restrict__ t2, const uint16_t* __restrict__ zpos,
+                                           int q, int npp)
+{
+    if constexpr (MT0 < add_nmt(NX)) {
+        constexpr int N0 = add_nks(NX, MT0);
+        constexpr int N1 = (MT0 + 1 < add_nmt(NX)) ? add_nks(NX, MT0 + 1 < add_nmt(NX) ? MT0 + 1 : MT0) : 0;
+        double d[2][2][2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) d[u][0][0] = d[u][0][1] = d[u][1][0] = d[u][1][1] = 0.0;
+        add_zpair<N0, N1, CPLX>(stg_lane + (size_t)BLK * 64, stg_lane + (size_t)(BLK + N0) * 64, fzl, phased, wr, wi, d);
+#pragma unroll
+        for (int u = 0; u < 2; ++u)
+            if (u == 0 || N1 > 0) {
+                double* o = t2 + zpos[8 * (MT0 + u) + q];
+                o[0] = d[u][0][0]; o[npp] = d[u][0][1];
+                o[(size_t)kAddTZ * npp] = d[u][1][0]; o[(size_t)kAddTZ * npp + npp] = d[u][1][1];
+            }
+        add_ztiles<NX, MT0 + 2, BLK + N0 + N1, CPLX>(stg_lane, fzl, phased, wr, wi, t2, zpos, q, npp);
+    }
+}
+
 // MIX (numax = 8, 9 only): the third K step of the y stage holds just ny = 8, 9, and the x stage spends one MMA per
 // channel on the three pairs (ny, nx) = (8,0), (8,1), (9,0) and another on (0,8), (0,9), (1,8).  With MIX the free
 // half of that y K step carries ny = 0, 1 a second time -- A fragment (phi_8, phi_9, phi_0, phi_1)(y) -- against the
 // partial x sums over nx = 8, 9 only, and ONE x-stage MMA with the A fragment (phi_0, phi_1, phi_8, phi_9)(x) yields
 // its four B columns: T1[x][8], T1[x][9] (from nx = 0, 1) and the nx = 8, 9 parts of T1[x][0], T1[x][1].  Three
 // x-stage MMAs per plane and channel instead of four, two shared-memory loads fewer; nothing else changes.
-// NX: the numax this variant is compiled for (8, 9), or -1: any numax with this KQ, sizes at run time
+// NX: the numax this variant is compiled for (5, 7, 8, 9: the configs' and the paper's), or -1: any numax with this KQ,
+// sizes at run time.  With NX the z stage is straight-line code (add_ztiles) instead of a loop over a jump table.
 template <int KQ, int DT, int NX>
 __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel(const __grid_constant__ AddParams p)
 {
@@ -655,6 +687,9 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
                 const double wr = en->wr, wi = en->wi;
                 const bool phased = !(wr == 1.0 && wi == 0.0);                  // warp-uniform; most images have none
                 double* t2 = T2 + (size_t)slot * T2S + (size_t)(2 * t) * npp;
+                if constexpr (EX) {
+                    add_ztiles<(EX ? NX : 0), 0, 0, CPLX>(stg + (size_t)lane * 2, fzw + lane, phased, wr, wi, t2, ZPOS, q, npp);
+                } else {
                 int blk_run = 0;                     // first K block of row tile mt0 (the tiles' blocks are consecutive)
                 for (int mt0 = 0; mt0 < nmt; mt0 += 2) {
                     double d[2][2][2];
@@ -687,6 +722,7 @@ __global__ void __launch_bounds__(add_threads(Elem<DT>::cplx), 1) sho_add_kernel
                             o[0] = d[u][0][0]; o[npp] = d[u][0][1];
                             o[(size_t)kAddTZ * npp] = d[u][1][0]; o[(size_t)kAddTZ * npp + npp] = d[u][1][1];
                         }
+                }
                 }
             }
             __syncwarp();
@@ -761,7 +797,9 @@ static sho_status launch_kq(const sho_plan* pl, const void* coeff, int nbands, v
 {
     switch ((pl->g.numax + 4) >> 2) {          // K steps of four n values that hold n <= numax
         case 1: return launch_t<1, DT, -1>(pl, coeff, nbands, psi, s, cnb, t1);
-        case 2: return launch_t<2, DT, -1>(pl, coeff, nbands, psi, s, cnb, t1);      // NX = 5, 7 measured: 1 % slower
+        case 2: return pl->g.numax == 7 ? launch_t<2, DT, 7>(pl, coeff, nbands, psi, s, cnb, t1)
+                     : pl->g.numax == 5 ? launch_t<2, DT, 5>(pl, coeff, nbands, psi, s, cnb, t1)
+                                        : launch_t<2, DT, -1>(pl, coeff, nbands, psi, s, cnb, t1);
         case 3: return pl->g.numax == 9 ? launch_t<3, DT, 9>(pl, coeff, nbands, psi, s, cnb, t1)
                      : pl->g.numax == 8 ? launch_t<3, DT, 8>(pl, coeff, nbands, psi, s, cnb, t1)
                                         : launch_t<3, DT, -1>(pl, coeff, nbands, psi, s, cnb, t1);
