@@ -48,7 +48,8 @@ static __device__ __noinline__ void mbar_wait_slow(uint32_t a, int parity)
 {
     const unsigned long long t0 = global_timer_ns();
     for (;;) {
-        for (int spin = 0; spin < 4096; ++spin)
+#pragma unroll 1
+        for (int spin = 0; spin < 4096; ++spin)          // a compact loop: unrolled, this cold path was 280 instructions
             if (mbar_try_wait(a, parity)) return;
         if (global_timer_ns() - t0 > kMbarTimeoutNs) __trap();
     }
