@@ -198,6 +198,35 @@ sho_status sho_add_bf(const sho_plan* plan, const void* coeff, int32_t nbands, v
                       void* cuda_stream);
 
 /*
+ * sho_project_bf for callers that cannot bring a workspace.  Same arguments, same result as sho_project_bf, but the
+ * chunks of bands are converted in a fixed workspace of SHO_STATIC_WORK_BYTES that is part of the library image
+ * instead of one the caller allocates.
+ *
+ * Who needs this: code that is handed psi and coeff by a host application and has no device memory of its own to
+ * lend -- a plug-in inside a DFT program that gave all of the GPU's memory to its own arena at start-up (cudaMalloc
+ * then fails), or a routine that is called while the application's other streams are busy (cudaMalloc and cudaFree
+ * synchronise the whole device and would stall them).  This call never calls cudaMalloc, cudaFree or any library
+ * routine that allocates; the plan it takes was created earlier, at a time when allocating was still possible.
+ *
+ * Limit: one band of the plan's grid, Nx*Ny*Nz*sizeof(element), must fit in SHO_STATIC_WORK_BYTES (32 MiB: e.g.
+ * 128^3 real fp64, the paper's 64^3 grid in every dtype); a larger grid returns SHO_ERR_UNSUPPORTED with the sizes in
+ * sho_last_error(), and nothing is launched.  As many bands per chunk as fit are used (the paper's 64^3 fp64
+ * grid: 16).
+ * Cost: every GPU on which the library's module is loaded holds these 32 MiB until the process exits, whether or
+ * not this function is ever called.
+ * First call: the first call on each device (with that device current) looks up the device address of the
+ * workspace (cudaGetSymbolAddress; this may make the runtime load the library's module) and caches it; make that
+ * first call during set-up, before any stream capture begins.
+ * Sharing: all calls on one device share the one workspace, which keeps whatever the last call left in it.  This
+ * entry point does not depend on those contents (each chunk is fully written before it is read), but two calls
+ * whose kernels can overlap on the GPU -- different streams, or different host threads on different streams --
+ * race on it and give wrong coefficients: keep all calls on one device on one stream, or order them with events.
+ * Asynchronous on the stream otherwise, like sho_project_bf.
+ */
+#define SHO_STATIC_WORK_BYTES (32u << 20)
+sho_status sho_project_bf_static(const sho_plan* plan, const void* psi_bf, int32_t nbands, void* coeff, void* cuda_stream);
+
+/*
  * End-to-end variants with HOST buffers (pinned or pageable): copy in, run the same kernels, copy
  * out, and synchronise the stream before returning.  They use a device workspace owned by the plan
  * (the only hot-path calls that may allocate; it is grown on demand and bounded by the chunk size, not

@@ -95,6 +95,7 @@ def lib():
     L.sho_add_stored1d.argtypes = [_vp, _vp, _vp, C.c_int32, _vp, _vp]
     L.sho_project_bf.argtypes = [_vp, _vp, C.c_int32, _vp, _vp, C.c_size_t, _vp]
     L.sho_add_bf.argtypes = [_vp, _vp, C.c_int32, _vp, _vp, C.c_size_t, _vp]
+    L.sho_project_bf_static.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
     L.sho_dmul.argtypes = [_vp, _vp, _vp, C.c_int32, _vp, _vp]
     L.sho_apply.argtypes = [_vp, _vp, _vp, C.c_int32, _vp, _vp]
     L.sho_apply_host.argtypes = [_vp, _vp, _vp, C.c_int32, _vp]
@@ -353,6 +354,20 @@ class Plan:
                                     work.numel() * work.element_size(), _stream_handle(stream)), "sho_project_bf")
         return coeff
 
+    def project_bf_static(self, psi_bf, coeff=None, stream=None):
+        """sho_project_bf without a workspace argument: the library converts the band chunks in its own fixed
+        32 MiB device array (STATIC_WORK_BYTES), so the C call allocates nothing.  Meant for callers that own only
+        psi_bf and coeff (see include/sho.h); pass ``coeff`` to keep this wrapper from allocating the output too.
+        Calls on one device share that array: keep them on one stream.  ShoError (SHO_ERR_UNSUPPORTED) if one band
+        of the grid is larger than the array."""
+        nb = self._check_psi_bf(psi_bf, "sho_project_bf_static")
+        if coeff is None:
+            coeff = self.new_coeff(nb, psi_bf.device)
+        self._check_coeff(coeff, nb, "sho_project_bf_static")
+        _check(lib().sho_project_bf_static(self._h, psi_bf.data_ptr(), nb, coeff.data_ptr(), _stream_handle(stream)),
+               "sho_project_bf_static")
+        return coeff
+
     def add_bf(self, coeff, psi_bf, work=None, stream=None):
         nb = self._check_psi_bf(psi_bf, "sho_add_bf")
         self._check_coeff(coeff, nb, "sho_add_bf")
@@ -489,6 +504,13 @@ def sho_project_bf(plan: Plan, psi_bf, coeff=None, work=None, stream=None):
 
 def sho_add_bf(plan: Plan, coeff, psi_bf, work=None, stream=None):
     return plan.add_bf(coeff, psi_bf, work, stream)
+
+
+STATIC_WORK_BYTES = 32 << 20        # SHO_STATIC_WORK_BYTES of include/sho.h
+
+
+def sho_project_bf_static(plan: Plan, psi_bf, coeff=None, stream=None):
+    return plan.project_bf_static(psi_bf, coeff, stream)
 
 
 def sho_transform(plan: Plan, umat, coeff, out=None, stream=None):
