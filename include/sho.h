@@ -119,6 +119,12 @@ sho_status sho_add(const sho_plan* plan, const void* coeff, int32_t nbands, void
  * sho_tables_build samples Phi_n(r - R_a) over every box into device memory (element type = the
  * real type of the plan's dtype).  *bytes_needed is always filled; if the tables do not fit in free
  * device memory the call returns SHO_ERR_OOM and *out = NULL.  Pass out = NULL to query the size only.
+ * sho_project_stored adds the partial sums of the box's z segments in a fixed order (bit-reproducible); the small
+ * hand-over counters it needs for that live in the tables object.  Calls that share one tables object may come from
+ * any stream or host thread: the library chains them on the device (each launch waits for the one before it on
+ * that object), so they are safe but do not overlap; use one tables object per stream to overlap them.  One call
+ * covers at most 256 groups of 32 real columns per atom, i.e. nbands <= 8192 (real) or 4096 (complex); more bands
+ * return SHO_ERR_UNSUPPORTED -- split the call (bands are independent).
  */
 sho_status sho_tables_build(const sho_plan* plan, sho_tables** out, size_t* bytes_needed, void* cuda_stream);
 sho_status sho_tables_destroy(sho_tables* tables);

@@ -476,6 +476,7 @@ sho_status sho_tables_destroy(sho_tables* t)
     cudaFree(t->d_seg_atom);
     cudaFree(t->d_seg_qz0);
     cudaFree(t->d_turn);
+    if (t->last_launch) cudaEventDestroy(t->last_launch);
     delete t;
     return SHO_OK;
 }
@@ -686,23 +687,32 @@ static sho_status host_run(sho_plan* plan, HostMode mode, const char* fn, void* 
     if (!plan->s_out && cudaStreamCreateWithFlags(&plan->s_out, cudaStreamNonBlocking) != cudaSuccess) return cuda_fail(cudaGetLastError(), fn);
     cudaStream_t s_in = plan->s_in, s_out = plan->s_out;
     std::vector<cudaEvent_t> events;
+    // Every ordering edge between the three streams is an event.  A failed event call would silently drop an edge
+    // (the streams would then race on the chunk buffers), so the first failure is kept in ev_err and ends the call.
+    cudaError_t ev_err = cudaSuccess;
+    auto note = [&](cudaError_t r) { if (r != cudaSuccess && ev_err == cudaSuccess) ev_err = r; return r == cudaSuccess; };
     auto mark = [&](cudaStream_t signaller) -> cudaEvent_t {                            // an event behind what signaller has queued
-        cudaEvent_t e = nullptr;
-        cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
-        events.push_back(e);
-        cudaEventRecord(e, signaller);
-        return e;
+        cudaEvent_t ev = nullptr;
+        if (!note(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming))) return nullptr;
+        events.push_back(ev);
+        if (!note(cudaEventRecord(ev, signaller))) return nullptr;
+        return ev;
     };
     // waiter continues after what signaller has queued (the caller's stream may be the default stream, handle 0)
-    auto after = [&](cudaStream_t waiter, cudaStream_t signaller) { cudaStreamWaitEvent(waiter, mark(signaller), 0); };
+    auto after = [&](cudaStream_t waiter, cudaStream_t signaller) {
+        cudaEvent_t ev = mark(signaller);
+        if (ev) note(cudaStreamWaitEvent(waiter, ev, 0));
+    };
     // on any failure: let everything that was queued finish before the caller gets its buffers back
     auto finish = [&](sho_status status) {
         cudaStreamSynchronize(s_in); cudaStreamSynchronize(s); cudaStreamSynchronize(s_out);
         for (cudaEvent_t e : events) cudaEventDestroy(e);
         return status;
     };
+    auto edge_lost = [&]() { return finish(cuda_fail(ev_err, fn)); };
     after(s_in, s);                         // the copies start after what the caller queued on its stream
     after(s_out, s);
+    if (ev_err != cudaSuccess) return edge_lost();
     cudaEvent_t slot_free[kHostRing] = { nullptr, nullptr, nullptr };
     cudaError_t e = cudaSuccess;
     for (int i = 0, b0 = 0; b0 < nbands; ++i, b0 += cb) {
@@ -711,7 +721,7 @@ static sho_status host_run(sho_plan* plan, HostMode mode, const char* fn, void* 
         char* d_c = static_cast<char*>(plan->ws_c) + (size_t)slot * c_slot;                 // [natoms][nb][N_SHO]
         char* h_psi = static_cast<char*>(psi_host) + (size_t)b0 * band_bytes;
         char* h_c = coeff_host ? static_cast<char*>(coeff_host) + (size_t)b0 * row_bytes : nullptr;
-        if (slot_free[slot]) cudaStreamWaitEvent(s_in, slot_free[slot], 0);
+        if (slot_free[slot] && !note(cudaStreamWaitEvent(s_in, slot_free[slot], 0))) return edge_lost();
         if (mode == kHostAdd && plan->g.natoms > 0) {
             e = cudaMemcpy2DAsync(d_c, (size_t)nb * row_bytes, h_c, (size_t)nbands * row_bytes, (size_t)nb * row_bytes,
                                   (size_t)plan->g.natoms, cudaMemcpyHostToDevice, s_in);
@@ -720,6 +730,7 @@ static sho_status host_run(sho_plan* plan, HostMode mode, const char* fn, void* 
         e = cudaMemcpyAsync(d_psi, h_psi, band_bytes * nb, cudaMemcpyHostToDevice, s_in);
         if (e != cudaSuccess) return finish(cuda_fail(e, fn));
         after(s, s_in);
+        if (ev_err != cudaSuccess) return edge_lost();
         if (plan->g.natoms > 0) {
             if (mode == kHostProject) st = launch_project(plan, d_psi, nb, d_c, s);
             else if (mode == kHostAdd) st = plan->n_tile_list ? launch_add(plan, d_c, nb, d_psi, s) : SHO_OK;
@@ -731,6 +742,7 @@ static sho_status host_run(sho_plan* plan, HostMode mode, const char* fn, void* 
             if (st != SHO_OK) return finish(st);
         }
         after(s_out, s);
+        if (ev_err != cudaSuccess) return edge_lost();
         if (mode == kHostProject) {
             if (plan->g.natoms > 0)
                 e = cudaMemcpy2DAsync(h_c, (size_t)nbands * row_bytes, d_c, (size_t)nb * row_bytes, (size_t)nb * row_bytes,
@@ -740,8 +752,10 @@ static sho_status host_run(sho_plan* plan, HostMode mode, const char* fn, void* 
         }
         if (e != cudaSuccess) return finish(cuda_fail(e, fn));
         slot_free[slot] = mark(s_out);
+        if (ev_err != cudaSuccess) return edge_lost();
     }
     after(s, s_out);
+    if (ev_err != cudaSuccess) return edge_lost();
     e = cudaStreamSynchronize(s);
     for (cudaEvent_t ev : events) cudaEventDestroy(ev);
     if (e != cudaSuccess) return cuda_fail(e, fn);

@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -113,8 +114,10 @@ struct sho_tables {
     int32_t* d_seg_atom;                   // K segments (atom, first box plane) = the CTAs of the stored kernel
     int32_t* d_seg_qz0;
     int32_t nseg;
-    int* d_turn;                           // [turn_count] turnstile counters of sho_project_stored (256 column groups per atom)
+    int* d_turn;                           // [1 + turn_count] work ticket, then the turnstile counters of sho_project_stored (256 column groups per atom)
     size_t turn_count;
+    cudaEvent_t last_launch;               // recorded behind every sho_project_stored launch; the next launch waits for it
+    mutable std::mutex launch_mutex;       // host side of that chain (the ABI hands the object out as const)
     std::vector<int64_t> atom_off;
     size_t bytes;
 };
