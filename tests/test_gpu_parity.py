@@ -300,7 +300,7 @@ def test_project_band_loop_of_a_cta(sho, bpc, monkeypatch):
         plan.close()
 
 
-@pytest.mark.parametrize("k,dtype", [(3, None), (4, None), (4, "r32"), (5, None), ("paper", "r64")])
+@pytest.mark.parametrize("k,dtype", [(3, None), (4, None), (4, "r32"), (5, None), ("paper", "r64"), ("paper", "r32")])
 def test_full_size_config_sampled(sho, k, dtype):
     """BASELINE.json config k at its full size, in the launch configuration bench.py times (all bands, device
     inputs from a seeded torch generator), sampled as SURVEY 8(d) asks:
@@ -379,6 +379,169 @@ def test_full_size_config_sampled(sho, k, dtype):
         gotp = psi[:, iz, iy, ix].cpu().numpy().astype(wide).T
         e = (np.abs(gotp - refp).max(axis=0) / np.abs(refp).max(axis=0)).max()
         assert e <= tol, "add parity at full size, random points of all bands: %.3e > %.1e" % (e, tol)
+    finally:
+        plan.close()
+
+
+def test_cfg2_at_its_stated_size_in_full(sho):
+    """"Parity: full at cfg 1-3".  Config 2 as BASELINE.json states it (96^3 periodic, 32 atoms, numax 5,
+    16 bands): project, stored project, add, stored-1D and stored add compared with the oracle on EVERY element."""
+    w = workloads.make(2)
+    assert w.ng == (96, 96, 96) and w.natoms == 32 and w.nbands == 16 and w.numax == 5
+    run_case(sho, w)
+
+
+def test_cfg3_projection_at_its_stated_size_in_full(sho):
+    """Config 3 as stated (128^3 periodic, 256 atoms, numax 7, 32 bands): all 8192 x 120 coefficients against the
+    oracle's direct sum (2e11 multiply-adds on the host cores, about a minute).  The add-back of this config is
+    covered by the sampled full-size test above (planes and points computed point-wise by the oracle)."""
+    import torch
+    w = workloads.make(3)
+    assert w.ng == (128, 128, 128) and w.natoms == 256 and w.nbands == 32 and w.numax == 7
+    plan = sho.plan_for(w)
+    try:
+        assert np.array_equal(plan.boxes(), _oracle_boxes(w)), "integer box ranges differ from the oracle"
+        psi = w.psi()
+        c_gpu = plan.project(_dev(psi))
+        torch.cuda.synchronize()
+        check_project(sho, w, psi, c_gpu.cpu().numpy(), TOL[w.dtype])
+    finally:
+        plan.close()
+
+
+def _atoms_touching(w, boxes, pts):
+    """Atoms whose box (any periodic image) contains at least one of the grid points pts[n][3] = (jx, jy, jz)."""
+    hit = np.ones((w.natoms, len(pts)), bool)
+    for d in range(3):
+        N = w.ng[d]
+        on_axis = np.zeros((w.natoms, len(pts)), bool)
+        for m in (-2, -1, 0, 1, 2) if w.periodic[d] else (0,):
+            i = pts[:, d][None, :] + m * N
+            on_axis |= (i >= boxes[:, d, 0][:, None]) & (i <= boxes[:, d, 1][:, None])
+        hit &= on_axis
+    return np.nonzero(hit.any(axis=1))[0]
+
+
+def test_apply_host_at_cfg5_full_size_with_the_natural_chunk_rule(sho, monkeypatch):
+    """sho_apply_host -- the call bench.py's end-to-end number is measured through -- at config 5's full size with the
+    library's own chunk rule (no SHO_HOST_CHUNK_BANDS: one 113 MB band per chunk, 64 chunks through the three-slot
+    ring).  The three steps of PAPER.md:187-190 are recomputed by the oracle for two bands at the points of one
+    8 x 64 x 8 block of the grid and of a 4 x 4 x 4 block around the cell corner (every image wraps there, Bloch
+    phases on all axes): project_pairs for every atom whose box touches those points, dmul, add_points_bands."""
+    import torch
+    monkeypatch.delenv("SHO_HOST_CHUNK_BANDS", raising=False)
+    w = workloads.make(5)
+    assert w.ng == (192, 192, 192) and w.natoms == 1024 and w.nbands == 64 and w.dtype == "c128"
+    plan = sho.plan_for(w)
+    try:
+        boxes = _oracle_boxes(w)
+        assert np.array_equal(plan.boxes(), boxes)
+        Nx, Ny, Nz = w.ng
+        bsel = [17, 63]
+        gen = torch.Generator(device="cuda")
+        gen.manual_seed(w.seed + 5)
+        host = torch.empty((w.nbands, Nz, Ny, Nx), dtype=torch.complex128, pin_memory=True)
+        bands = {}
+        for b in range(w.nbands):
+            band = torch.randn((Nz, Ny, Nx), dtype=torch.complex128, device="cuda", generator=gen)
+            host[b].copy_(band)
+            if b in bsel:
+                bands[b] = band.cpu().numpy()
+        del band
+        torch.cuda.synchronize()
+        Dm = w.dmatrix(plan.nsho)
+        plan.apply_host(Dm, host)
+        # ---- the oracle on the sampled points ----
+        blk = np.stack(np.meshgrid(np.arange(40, 48), np.arange(64, 128), np.arange(16, 24), indexing="ij"), -1).reshape(-1, 3)
+        edge = np.array([Nx - 2, Nx - 1, 0, 1])
+        cor = np.stack(np.meshgrid(edge, edge, edge, indexing="ij"), -1).reshape(-1, 3)
+        pts = np.concatenate([blk, cor]).astype(np.int32)
+        atoms = _atoms_touching(w, boxes, pts)
+        assert 20 <= len(atoms) <= 400
+        pa = np.repeat(atoms, len(bsel))
+        pb = np.tile(np.array(bsel), len(atoms))
+        geo = (w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax)
+        c = oracle.project_pairs(*geo, bands, pa, pb, w.nbands, True, w.rcut_sigma)             # [pairs][N_SHO]
+        c = c.reshape(len(atoms), len(bsel), plan.nsho)
+        d = oracle.dmul(np.ascontiguousarray(Dm[atoms]), c)
+        coeff = np.zeros((w.natoms, w.nbands, plan.nsho), np.complex128)                       # atoms that do not touch
+        coeff[np.ix_(atoms, bsel)] = d                                                         # the points add nothing there
+        inc = oracle.add_points_bands(*geo, coeff, pts, bsel, w.rcut_sigma)                      # [npts][2]
+        for i, b in enumerate(bsel):
+            ref = bands[b][pts[:, 2], pts[:, 1], pts[:, 0]] + inc[:, i]
+            got = host[b].numpy()[pts[:, 2], pts[:, 1], pts[:, 0]]
+            assert np.abs(inc[:, i]).max() > 1e-3 * np.abs(ref).max()                           # the action did something
+            err = np.abs(got - ref).max() / np.abs(ref).max()
+            assert err <= 1e-12, "sho_apply_host at cfg 5, band %d: %.3e > 1e-12" % (b, err)
+    finally:
+        plan.close()
+
+
+def test_dmul_and_transform_at_cfg5_full_size_in_full(sho):
+    """Step (2) d = D c and the spherical transform (eq. (10)-(11)) on all of config
+    5's 1024 x 64 x 220 complex coefficients against oracle.dmul, every element."""
+    import torch
+    w = workloads.make(5)
+    plan = sho.plan_for(w)
+    try:
+        rng = np.random.default_rng(55)
+        D = rng.standard_normal((w.natoms, plan.nsho, plan.nsho)) / np.sqrt(plan.nsho)           # not symmetric
+        c = w.coeff(plan.nsho)
+        ref = oracle.dmul(D, c)
+        d_c = _dev(c)
+        out = plan.dmul(_dev(D), d_c)
+        torch.cuda.synchronize()
+        assert np.abs(out.cpu().numpy() - ref).max() <= 1e-12 * np.abs(ref).max()
+        del out, D
+        Uo = oracle.umatrix(w.numax)
+        ref = oracle.dmul(np.ascontiguousarray(np.broadcast_to(Uo, (w.natoms,) + Uo.shape)), c)
+        out = plan.transform(_dev(sho.umatrix(w.numax)), d_c)
+        torch.cuda.synchronize()
+        assert np.abs(out.cpu().numpy() - ref).max() <= 1e-12 * np.abs(ref).max()
+    finally:
+        plan.close()
+
+
+def test_band_fastest_layout_at_the_papers_full_size(sho):
+    """sho_project_bf / sho_add_bf on the paper's own workload at full size (64^3, 665 atoms, 1024 bands, psi_bf of
+    2.1 GB, chunks of 64 bands): sampled (atom, band) pairs against the oracle's direct sum, and the add-back at 2048
+    random points of ALL bands computed point-wise by the oracle."""
+    import torch
+    w = workloads.make_paper(5, "r64")
+    plan = sho.plan_for(w)
+    try:
+        boxes = _oracle_boxes(w)
+        gen = torch.Generator(device="cuda")
+        gen.manual_seed(w.seed + 1)
+        psi = torch.randn((w.nbands, w.ng[2], w.ng[1], w.ng[0]), dtype=torch.float64, device="cuda", generator=gen)
+        psi_bf = psi.permute(1, 2, 3, 0).contiguous()
+        c_bf = plan.project_bf(psi_bf)
+        torch.cuda.synchronize()
+        atoms = _sample_atoms(w, boxes)
+        bsel = _sample_bands(w.nbands)
+        pa = np.repeat(np.array(atoms), len(bsel))
+        pb = np.tile(np.array(bsel), len(atoms))
+        bands = {b: psi[b].cpu().numpy() for b in bsel}
+        ref = oracle.project_pairs(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax, bands, pa, pb, w.nbands,
+                                   False, w.rcut_sigma)
+        norm = np.array([np.sqrt(w.h ** 3 * np.sum(bands[int(b)] ** 2)) for b in pb])
+        got = c_bf[torch.as_tensor(pa, device="cuda"), torch.as_tensor(pb, device="cuda")].cpu().numpy()
+        err = (np.abs(got - ref) / norm[:, None]).max()
+        assert err <= 1e-12, "sho_project_bf at the paper's full size: %.3e" % err
+        coeff = torch.randn((w.natoms, w.nbands, plan.nsho), dtype=torch.float64, device="cuda", generator=gen)
+        del psi
+        before = psi_bf.clone()
+        plan.add_bf(coeff, psi_bf)
+        torch.cuda.synchronize()
+        rng = np.random.default_rng(w.seed)
+        pts = np.stack([rng.integers(0, w.ng[d], 2048) for d in range(3)], axis=1)
+        inc = oracle.add_points_bands(w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax, coeff.cpu().numpy(), pts,
+                                      np.arange(w.nbands), w.rcut_sigma)                          # [npts][nbands]
+        iz, iy, ix = (torch.as_tensor(pts[:, d], device="cuda") for d in (2, 1, 0))
+        refp = before[iz, iy, ix].cpu().numpy() + inc
+        gotp = psi_bf[iz, iy, ix].cpu().numpy()
+        e = (np.abs(gotp - refp).max(axis=0) / np.abs(refp).max(axis=0)).max()
+        assert e <= 1e-12, "sho_add_bf at the paper's full size: %.3e" % e
     finally:
         plan.close()
 
@@ -553,6 +716,35 @@ def test_stored_projection_is_bit_reproducible(sho):
     tb.close()
     plan.close()
     assert all(torch.equal(outs[0], o) for o in outs[1:])
+
+
+def test_stored_projections_sharing_one_tables_object_on_two_streams(sho):
+    """The hand-over counters of sho_project_stored live in the tables object: launches that share it are chained on
+    the device by the library, so issuing them on two streams at once must give what one stream gives (bit for bit),
+    not a race on the counters (wrong sums or a hang)."""
+    import torch
+    w = workloads.make(2)                                  # full size: 3.3 GB of tables, kernels of about a millisecond
+    plan = sho.plan_for(w)
+    psi_a = _dev(w.psi())
+    psi_b = psi_a.flip(0).contiguous()                     # the same bands in another order: other data per launch
+    tb = plan.tables()
+    try:
+        ref_a = plan.project_stored(tb, psi_a).clone()
+        ref_b = plan.project_stored(tb, psi_b).clone()
+        torch.cuda.synchronize()
+        assert torch.equal(ref_a, ref_b.flip(1))
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        outs_a = [plan.new_coeff(w.nbands, psi_a.device) for _ in range(6)]
+        outs_b = [plan.new_coeff(w.nbands, psi_a.device) for _ in range(6)]
+        for oa, ob in zip(outs_a, outs_b):
+            plan.project_stored(tb, psi_a, oa, stream=s1)
+            plan.project_stored(tb, psi_b, ob, stream=s2)
+        torch.cuda.synchronize()
+        assert all(torch.equal(ref_a, o) for o in outs_a)
+        assert all(torch.equal(ref_b, o) for o in outs_b)
+    finally:
+        tb.close()
+        plan.close()
 
 
 def test_host_buffer_entry_points(sho):

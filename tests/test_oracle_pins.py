@@ -615,6 +615,32 @@ def test_umatrix_textbook_shells(golden):
         assert U5[oracle.rlm_index(int(nr), int(l), int(m), 5), oracle.index(int(nx), int(ny), int(nz), 5)] == pytest.approx(float(v), abs=1e-14)
 
 
+def test_umatrix_f_shell_rows_from_harmonic_polynomials(golden):
+    """The whole f shell (l = 3, every m), the p* states and three g states against values that follow from the
+    mathematics alone (tests/golden/umatrix_harmonic_polynomials.txt: integer coefficients of the textbook solid
+    harmonics; U = p sqrt(a! b! c!) / norm).  An l-dependent sign slip or a wrong m order in the oracle's real
+    spherical harmonics -- which orthogonality and the block structure would not notice -- fails here: f_xyz must be
+    exactly the state |1 1 1>."""
+    import math
+    numax = 4
+    U = oracle.umatrix(numax)
+    rows = {}
+    for nr, l, m, a, b, c, p in golden("umatrix_harmonic_polynomials.txt"):
+        key = (int(nr), int(l), int(m))
+        abc = (int(a), int(b), int(c))
+        assert sum(abc) == key[1] + 2 * key[0]                                      # eq. (11): same shell
+        rows.setdefault(key, {})[abc] = int(p) * math.sqrt(math.factorial(abc[0]) * math.factorial(abc[1]) * math.factorial(abc[2]))
+    assert {k for k in rows if k[1] == 3} == {(0, 3, m) for m in range(-3, 4)}
+    for (nr, l, m), wts in rows.items():
+        norm = math.sqrt(sum(v * v for v in wts.values()))
+        want = np.zeros(U.shape[1])
+        for abc, v in wts.items():
+            want[oracle.index(*abc, numax)] = v / norm
+        got = U[oracle.rlm_index(nr, l, m, numax)]
+        assert np.max(np.abs(got - want)) < 1e-14, (nr, l, m)
+    assert U[oracle.rlm_index(0, 3, -2, numax), oracle.index(1, 1, 1, numax)] == pytest.approx(1.0, abs=1e-14)
+
+
 @pytest.mark.parametrize("numax", [0, 1, 3, 6])
 def test_umatrix_is_orthogonal_and_block_diagonal_in_nu(numax):
     """Unitarity ("a unitary transform") and eq. (11): elements vanish unless l + 2 nr = nx + ny + nz."""
