@@ -7,7 +7,9 @@ A step is one pass of the whole hot path over one batch of synthetic input: c = 
 followed by psi' += sho_add(c).  ``value`` is psi-GB/s(box): the bytes of every atom's psi box
 (read once by project, read + written once by add: 3 * sum_a |box_a| * nbands * sizeof(elem)) divided
 by the device time of the step, inputs resident in HBM.  ``e2e`` is the same metric through the
-HOST-buffer C-ABI calls (sho_project_host / sho_add_host), copies inside the timed region.
+HOST-buffer C-ABI call sho_apply_host (project -> D c -> add; psi crosses the link once each way), copies inside the
+timed region, beside the link rates measured in the same run; ``e2e.project_host_plus_add_host`` keeps round 1's
+definition (sho_project_host then sho_add_host).
 ``--impl reference`` times the CPU oracle (oracle/, test infrastructure) on a bounded sample.
 See DESIGN.md "Measurement" for every definition used here.
 """
@@ -47,17 +49,28 @@ def measured_peaks():
 
 
 def committed_traffic(workload, dtype, kernel):
-    """dram__bytes_read + dram__bytes_write of one launch from the committed ncu --set full capture of this
-    workload and kernel (profiles/traffic.json, written from the .ncu-rep named there), or None."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
-    if not os.path.exists(path):
-        return None, None
-    with open(path) as f:
-        t = json.load(f)
-    e = t.get("%s/%s/%s" % (workload, dtype, kernel))
-    if not e:
-        return None, None
-    return float(e["dram_bytes_read"]) + float(e["dram_bytes_write"]), "profiles/traffic.json <- %s" % e.get("source", "?")
+    """dram__bytes_read + dram__bytes_write of one launch of ``kernel``, read from the committed summary of the
+    ncu --set full capture of this workload (profiles/r<N>_final_<workload>_ncu_full.txt, the latest round that has
+    one; its first line names the element type, its second the command).  (None, None) if there is no capture."""
+    import glob
+    import re
+    unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_final_%s_ncu_full.txt" % workload)), reverse=True):
+        with open(path) as f:
+            lines = f.read().splitlines()
+        if not lines or dtype not in lines[0]:
+            continue
+        cur, found = None, {}
+        for ln in lines:
+            if ln.startswith("kernel:"):
+                cur = ln
+            elif cur and re.search(r"\b%s\b" % re.escape(kernel), cur):
+                m = re.match(r"\s*dram__bytes_(read|write)\.sum\s+(\w+)\s+([0-9.eE+-]+)\s*$", ln)
+                if m and m.group(2) in unit and m.group(1) not in found:
+                    found[m.group(1)] = float(m.group(3)) * unit[m.group(2)]
+        if len(found) == 2:
+            return found["read"] + found["write"], "%s (ncu --set full, one launch)" % os.path.relpath(path, ROOT)
+    return None, None
 
 
 def geometry(w, boxes=None):
@@ -231,6 +244,9 @@ def stored_vs_on_the_fly(sho, torch, dev, w3, steps):
     t_fly = med(lambda: plan.project(psi, coeff, stream))
     t_sto = med(lambda: plan.project_stored(tb, psi, coeff, stream))
     tb.close()
+    psi.zero_()
+    t_add = med(lambda: plan.add(coeff, psi, stream))
+    out["ms_add_on_the_fly"] = 1e3 * t_add
     plan.close()
     peaks, _ = measured_peaks()
     P = g3["P"]
@@ -335,14 +351,18 @@ def run_ours(args, w):
     # ---- the three-step action project -> D -> add in one call (f2), device resident, outside the timed region ----
     dmat = torch.from_numpy(w.dmatrix(plan.nsho)).to(dev)
     plan.apply(dmat, psi_out, coeff, stream)
-    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
-    e0.record(stream)
-    plan.dmul(dmat, coeff, coeff, stream)
-    e1.record(stream)
-    plan.apply(dmat, psi_out, coeff, stream)
-    e2.record(stream)
+    ka = max(3, min(args.steps, 5))                                   # medians, like the per-kernel times above
+    eva = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(ka)]
+    for e0, e1, e2 in eva:
+        psi_out.zero_()                                               # keeps psi finite over repeated applications
+        e0.record(stream)
+        plan.dmul(dmat, coeff, coeff, stream)
+        e1.record(stream)
+        plan.apply(dmat, psi_out, coeff, stream)
+        e2.record(stream)
     torch.cuda.synchronize()
-    t_dmul, t_apply = e0.elapsed_time(e1) * 1e-3, e1.elapsed_time(e2) * 1e-3
+    t_dmul = float(np.median([e[0].elapsed_time(e[1]) for e in eva])) * 1e-3
+    t_apply = float(np.median([e[1].elapsed_time(e[2]) for e in eva])) * 1e-3
     psi_out.zero_()
 
     # ---- end to end through the HOST-buffer C-ABI call sho_apply_host (pinned host memory): psi is uploaded once,
@@ -367,6 +387,50 @@ def run_ours(args, w):
         e2e = {"value": step_bytes * ke / te / 1e9, "unit": "GB/s", "h2d_bytes_per_step": psi_b + d_b,
                "d2h_bytes_per_step": psi_b, "steps": ke, "ms_per_step": 1e3 * te / ke,
                "call": "sho_apply_host (project -> D c -> add, one upload and one download of psi per step)"}
+        # the host link measured in the same run: pinned H2D and D2H copies of up to 2 GB each, at the same time on two
+        # streams (the pattern of the chunk pipeline); the step's link bound is the slower direction's bytes / rate
+        nlink = min(psi_b, 2 << 30)
+        src_h = hp.view(torch.uint8).reshape(-1)[:nlink]
+        dst_h = torch.empty(nlink, dtype=torch.uint8, pin_memory=True)
+        dev_a = torch.empty(nlink, dtype=torch.uint8, device=dev)
+        dev_b = torch.empty(nlink, dtype=torch.uint8, device=dev)
+        sa, sb = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+        rates = []
+        for _ in range(3):                                               # the first pass is a warm-up
+            torch.cuda.synchronize()
+            ea0, ea1, eb0, eb1 = (torch.cuda.Event(enable_timing=True) for _ in range(4))
+            with torch.cuda.stream(sa):
+                ea0.record(sa); dev_a.copy_(src_h, non_blocking=True); ea1.record(sa)
+            with torch.cuda.stream(sb):
+                eb0.record(sb); dst_h.copy_(dev_b, non_blocking=True); eb1.record(sb)
+            torch.cuda.synchronize()
+            rates.append((nlink / (ea0.elapsed_time(ea1) * 1e-3) / 1e9, nlink / (eb0.elapsed_time(eb1) * 1e-3) / 1e9))
+        h2d_gbs, d2h_gbs = max(r[0] for r in rates[1:]), max(r[1] for r in rates[1:])
+        link_bound = max((psi_b + d_b) / (h2d_gbs * 1e9), psi_b / (d2h_gbs * 1e9))
+        e2e.update(pcie_h2d_gbs=h2d_gbs, pcie_d2h_gbs=d2h_gbs, link_bound_ms=1e3 * link_bound,
+                   frac_of_link_bound=link_bound / (te / ke),
+                   link_note="pinned H2D and D2H measured concurrently in this run; bound = max(h2d bytes / h2d rate, d2h bytes / d2h rate)")
+        del src_h, dst_h, dev_a, dev_b
+        # the round-1 end-to-end leg, kept so that the series stays comparable: sho_project_host (psi up, c down) followed
+        # by sho_add_host (c and psi up, psi down)
+        if w.natoms > 0:
+            hc = torch.empty((w.natoms, nb, plan.nsho), dtype=tdt, pin_memory=True)
+            hp.copy_(psi)
+            plan.project_host(hp, hc, stream)
+            hp.zero_()
+            plan.add_host(hc, hp, stream)                                 # warm-up of both calls
+            barrier()
+            t0 = time.perf_counter()
+            plan.project_host(hp, hc, stream)
+            plan.add_host(hc, hp, stream)
+            torch.cuda.synchronize()
+            tpa = time.perf_counter() - t0
+            (tpa,) = sharding.max_over_ranks([tpa], device=dev)
+            c_b = w.natoms * nb * plan.nsho * esz
+            e2e["project_host_plus_add_host"] = {"value": step_bytes / tpa / 1e9, "unit": "GB/s", "ms_per_step": 1e3 * tpa,
+                                                 "h2d_bytes_per_step": 2 * psi_b + c_b, "d2h_bytes_per_step": psi_b + c_b,
+                                                 "note": "the e2e definition of BENCH_r01 (two calls, psi crosses the link three times)"}
+            del hc
         del hp, hd
 
     if rank != 0:
@@ -428,6 +492,12 @@ def run_ours(args, w):
         del psi_out
         torch.cuda.empty_cache()
         stored_cfg3 = stored_vs_on_the_fly(sho, torch, dev, workloads.make(3), min(args.steps, 5))
+    # the paper's own benchmark (sec. 6, tab. 1: 64^3, 665 atoms, 1024 bands, 56 coefficients, double) as a
+    # sub-leg of the default run, outside the timed region: on-the-fly project / add and the stored-projector projection
+    paper_nu5 = None
+    if not args.no_stored and not w.name.startswith("paper") and world == 1:
+        torch.cuda.empty_cache()
+        paper_nu5 = stored_vs_on_the_fly(sho, torch, dev, workloads.make_paper(5, "r64"), min(args.steps, 5))
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         s = oracle_sample_setup(w, cpu_seconds=args.ref_cpu_seconds)
@@ -455,7 +525,7 @@ def run_ours(args, w):
             "atom_band_per_s": world * info["atoms_nonempty"] * nb * args.steps / t_total,
             "tflops_project": F / t_prj / 1e12, "tflops_add": F / t_add / 1e12, "fp64_peak_measured_tflops": fp64_meas,
             "ms_dmul": 1e3 * t_dmul, "ms_apply_project_dmul_add": 1e3 * t_apply,
-            "stored_baseline": stored, "stored_baseline_cfg3": stored_cfg3, "separable_stored1d": sep1d, "sum_box_points": g["sum_box"], "psi_bytes_unique": int(np.prod(shape)) * esz, "add_tile_pairs": info["add_pairs"],
+            "stored_baseline": stored, "stored_baseline_cfg3": stored_cfg3, "paper_nu5": paper_nu5, "pcie_gbs": ({"h2d": e2e["pcie_h2d_gbs"], "d2h": e2e["pcie_d2h_gbs"]} if e2e else None), "separable_stored1d": sep1d, "sum_box_points": g["sum_box"], "psi_bytes_unique": int(np.prod(shape)) * esz, "add_tile_pairs": info["add_pairs"],
         },
     }
     print(json.dumps(line))

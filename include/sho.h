@@ -92,6 +92,16 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
                            int32_t numax, double rcut_sigma, sho_dtype dtype);
 sho_status sho_plan_destroy(sho_plan* plan);
 
+/*
+ * Tuning / test knobs of one plan.  They change launch shapes only, never results (the tests check bit identity).
+ *   "project_bands_per_cta"  bands one CTA of sho_project works through with the tables it sampled once, 1..8;
+ *                            0 = chosen per launch from the band count and the grid size (default)
+ *   "host_chunk_bands"       bands per chunk of the *_host calls, >= 1; 0 = about 128 MB of psi per chunk (default)
+ * SHO_ERR_INVALID_ARG for an unknown key or a value out of range.  Set options before the plan is used by hot calls
+ * that may run at the same time on other host threads.
+ */
+sho_status sho_plan_set_option(sho_plan* plan, const char* key, int64_t value);
+
 /* test hook: integer box ranges, HOST lo_hi[natoms][3][2] = (i_lo, i_hi) per axis (unwrapped) */
 sho_status sho_plan_boxes(const sho_plan* plan, int32_t* lo_hi);
 
@@ -103,8 +113,8 @@ sho_status sho_plan_info(const sho_plan* plan, int64_t info[8]);
  * Projection, on-the-fly SHO.  psi DEVICE [nbands][Nz][Ny][Nx]; coeff DEVICE [natoms][nbands][N_SHO]
  * (overwritten; atoms with an empty box get zeros).  cuda_stream is a cudaStream_t (NULL = default).
  * Deterministic (fixed summation order, no atomics).  One CTA projects one atom and 1..8 consecutive bands
- * (chosen per launch from the band count and the grid size; the environment variable
- * SHO_PROJECT_BANDS_PER_CTA overrides it -- a test knob, the result does not depend on it).
+ * (chosen per launch from the band count and the grid size; sho_plan_set_option "project_bands_per_cta" overrides
+ * it -- a test knob, the result does not depend on it).
  */
 sho_status sho_project(const sho_plan* plan, const void* psi, int32_t nbands, void* coeff, void* cuda_stream);
 
@@ -237,7 +247,7 @@ sho_status sho_project_bf_static(const sho_plan* plan, const void* psi_bf, int32
  * out, and synchronise the stream before returning.  They use a device workspace owned by the plan
  * (the only hot-path calls that may allocate; it is grown on demand and bounded by the chunk size, not
  * by nbands).  The bands are independent (eq. (25)), so the calls work in chunks of bands
- * (about 128 MB of psi each; environment variable SHO_HOST_CHUNK_BANDS overrides the chunk size)
+ * (about 128 MB of psi each; sho_plan_set_option "host_chunk_bands" overrides the chunk size)
  * through a ring of three chunk buffers and overlap the H2D copy of the next chunk, the kernels of this
  * one and the D2H copy of the previous one on two copy streams owned by the plan; all of it is ordered
  * after the work already queued on cuda_stream.  If a step fails mid-way the call waits for everything

@@ -75,6 +75,7 @@ def lib():
     L.sho_plan_create.argtypes = [C.POINTER(_vp), _i32p, C.c_double, _i32p, _f64p, C.c_int32, _f64p, _f64p,
                                   C.c_int32, C.c_double, C.c_int]
     L.sho_plan_destroy.argtypes = [_vp]
+    L.sho_plan_set_option.argtypes = [_vp, C.c_char_p, C.c_int64]
     L.sho_plan_boxes.argtypes = [_vp, _i32p]
     L.sho_plan_info.argtypes = [_vp, _i64p]
     L.sho_project.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
@@ -267,6 +268,11 @@ class Plan:
         torch = _torch()
         return torch.empty((self.natoms, int(nbands), self.nsho), dtype=_torch_dtype(self.dtype),
                            device=device or torch.device("cuda", torch.cuda.current_device()))
+
+    def set_option(self, key: str, value: int):
+        """Tuning / test knob of this plan (include/sho.h: "project_bands_per_cta", "host_chunk_bands"; 0 = automatic)."""
+        _check(lib().sho_plan_set_option(self._h, key.encode(), int(value)), "sho_plan_set_option")
+        return self
 
     # -- the hot calls ---------------------------------------------------------------------------
     def project(self, psi, coeff=None, stream=None):

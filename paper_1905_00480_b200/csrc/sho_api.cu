@@ -130,6 +130,7 @@ sho_status sho_plan_create(sho_plan** out, const int32_t ng[3], double h, const 
     p->d_tile_ptr = nullptr; p->d_tile_ent = nullptr; p->d_tile_list = nullptr; p->d_tile_info = nullptr; p->d_cainv = nullptr; p->d_t2pos = nullptr; p->d_cidx = nullptr;
     p->ws_psi = nullptr; p->ws_c = nullptr; p->ws_d = nullptr; p->ws_psi_bytes = 0; p->ws_c_bytes = 0; p->ws_d_bytes = 0;
     p->s_in = nullptr; p->s_out = nullptr;
+    p->opt_project_bands_per_cta = 0; p->opt_host_chunk_bands = 0;
     p->rcut_sigma = rcut_sigma;
     p->dtype = dtype;
     {
@@ -444,6 +445,23 @@ static sho_status check_hot(const char* fn, const sho_plan* plan, const void* a,
     return SHO_OK;
 }
 
+sho_status sho_plan_set_option(sho_plan* plan, const char* key, int64_t value)
+{
+    if (!plan || !key) { set_error("sho_plan_set_option: null argument"); return SHO_ERR_INVALID_ARG; }
+    if (std::strcmp(key, "project_bands_per_cta") == 0) {
+        if (value < 0 || value > 8) { set_error("sho_plan_set_option: project_bands_per_cta must be 0 (automatic) or 1..8"); return SHO_ERR_INVALID_ARG; }
+        plan->opt_project_bands_per_cta = (int32_t)value;
+        return SHO_OK;
+    }
+    if (std::strcmp(key, "host_chunk_bands") == 0) {
+        if (value < 0 || value > 0x7fffffff) { set_error("sho_plan_set_option: host_chunk_bands must be 0 (automatic) or >= 1"); return SHO_ERR_INVALID_ARG; }
+        plan->opt_host_chunk_bands = (int32_t)value;
+        return SHO_OK;
+    }
+    set_error("sho_plan_set_option: unknown key '%s'", key);
+    return SHO_ERR_INVALID_ARG;
+}
+
 sho_status sho_project(const sho_plan* plan, const void* psi, int32_t nbands, void* coeff, void* cuda_stream)
 {
     if (plan && plan->g.natoms == 0 && psi && nbands > 0) return SHO_OK;   // coeff is empty (may be null)
@@ -651,10 +669,7 @@ static sho_status ws_reserve(void** ws, size_t* have, size_t need, const char* w
 // number (the add kernel pairs real bands), at most 64 chunks
 static int host_chunk_bands(const sho_plan* plan, int nbands)
 {
-    if (const char* env = std::getenv("SHO_HOST_CHUNK_BANDS")) {            // tuning / test knob
-        const int v = std::atoi(env);
-        if (v > 0) return std::min(v, nbands);
-    }
+    if (plan->opt_host_chunk_bands > 0) return std::min(plan->opt_host_chunk_bands, nbands);   // sho_plan_set_option
     const double band_bytes = (double)plan->g.ng[0] * plan->g.ng[1] * plan->g.ng[2] * elem_size(plan->dtype);
     int cb = (int)std::max(1.0, std::floor(128.0e6 / band_bytes));
     cb = std::max(cb, (nbands + 63) / 64);

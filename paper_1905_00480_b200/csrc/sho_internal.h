@@ -104,6 +104,9 @@ struct sho_plan {
     void* ws_c;   size_t ws_c_bytes;
     void* ws_d;   size_t ws_d_bytes;       // atomic matrices of sho_apply_host
     cudaStream_t s_in, s_out;              // copy streams of the *_host calls (created on first use)
+    // sho_plan_set_option (0 = automatic)
+    int32_t opt_project_bands_per_cta;
+    int32_t opt_host_chunk_bands;
 };
 
 struct sho_tables {
@@ -114,7 +117,7 @@ struct sho_tables {
     int32_t* d_seg_atom;                   // K segments (atom, first box plane) = the CTAs of the stored kernel
     int32_t* d_seg_qz0;
     int32_t nseg;
-    int* d_turn;                           // [1 + turn_count] work ticket, then the turnstile counters of sho_project_stored (256 column groups per atom)
+    int* d_turn;                           // [turn_count] turnstile counters of sho_project_stored (256 column groups per atom)
     size_t turn_count;
     cudaEvent_t last_launch;               // recorded behind every sho_project_stored launch; the next launch waits for it
     mutable std::mutex launch_mutex;       // host side of that chain (the ABI hands the object out as const)

@@ -12,7 +12,7 @@
 //       8 rows x 128 B.  The loaded registers ARE the B fragments of the first contraction (K = x,
 //       N = 8 rows), so no shared-memory staging or transposition is needed, and the L1 data pipe moves
 //       a full line per wavefront (the earlier K = y layout touched 16 lines per 512 B and was bound by
-//       that pipe: profiles/r1_v2_cfg5_project_ncu_full.txt).  Periodic wrap / isolated clipping are
+//       that pipe, measured in round 1).  Periodic wrap / isolated clipping are
 //       per-lane index arithmetic from two small offset tables.  The loads run one group of G steps
 //       ahead of the arithmetic (register double buffer) and the ring runs on across row-block ends and
 //       plane ends, so loads stay in flight over the y stage, a5 and its barrier.
@@ -24,8 +24,9 @@
 //       second DMMA against the phi_ny table (the K order inside an MMA is free).  For R = 2 the six
 //       (nx,ny) outputs with nx or ny in {8, 9} are DFMA partials per lane.
 //   a5  third axis: each warp owns one z-plane per round; the per-plane T2[nx][ny] meet in shared
-//       memory and thread n accumulates c[n] += phi_nz(z) * T2[nx][ny] in a register.  One
-//       __syncthreads per round (double-buffered), coalesced store of N_SHO coefficients at the end.
+//       memory and thread n accumulates c[n] += phi_nz(z) * T2[nx][ny] in a register.  The T2
+//       planes go through four mbarrier-guarded buffers, the consumers one round behind the producers (no
+//       __syncthreads in the round loop); coalesced store of N_SHO coefficients at the end.
 // Bloch phases never touch the inner loop: the x-phase is one accumulator rotation at the wrap column,
 // y-phases rotate the a3 accumulators per row, the z-phase (and the last x image) is folded into a5.
 #include <algorithm>
@@ -639,10 +640,8 @@ static sho_status launch_t(const sho_plan* pl, const void* psi, int nbands, void
     const long long by_l2 = std::max<long long>(1, (long long)(24.0e6 / band_bytes));
     int bpc = (int)std::min<long long>(std::min<long long>(8, by_l2),
                                              std::max<long long>(1, (long long)pl->n_nonempty * nbands / (20 * per_wave)));
-    if (const char* env = std::getenv("SHO_PROJECT_BANDS_PER_CTA")) {      // test knob: the band loop on small inputs
-        const int v = std::atoi(env);
-        if (v >= 1) bpc = std::min(v, std::max(nbands, 1));
-    }
+    if (pl->opt_project_bands_per_cta >= 1)                                // sho_plan_set_option: the band loop on small inputs
+        bpc = std::min((int)pl->opt_project_bands_per_cta, std::max(nbands, 1));
     p.bands_per_cta = bpc;
     const long long nblocks = (long long)pl->n_nonempty * ((nbands + bpc - 1) / bpc);
     if (nblocks > 0x7fffffffLL) { set_error("sho_project: natoms*nbands too large"); return SHO_ERR_UNSUPPORTED; }

@@ -76,7 +76,6 @@ struct StoParams {
     int32_t nbands;
     long long band_stride;
     int* turn;                   // [natoms][ngroups] turnstile of the stored projection's K segments
-    unsigned* ticket;            // work items handed out so far in this launch (zeroed by the launcher)
     int32_t ngroups;
 };
 
@@ -92,14 +91,13 @@ __global__ void __launch_bounds__(kStoWarps * 32, 2) sho_project_stored_kernel(c
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int q = lane >> 2, t = lane & 3;
-    // Work items (K segment, column group) are handed out by a ticket taken when the CTA starts, not by blockIdx: the
-    // CTA that holds item w - 1 has then provably started, whatever order the hardware dispatches blocks in, so the
-    // turnstile wait at the end of the kernel (item w waits for w - 1 of the same atom) cannot wait for a CTA that
-    // is not resident.
-    __shared__ unsigned s_ticket;
-    if (tid == 0) s_ticket = atomicAdd(p.ticket, 1u);
-    __syncthreads();
-    const int seg = (int)(s_ticket % (unsigned)p.nseg), bg = (int)(s_ticket / (unsigned)p.nseg);
+    // Work item (K segment, column group) = block index.  The turnstile at the end of the kernel (segment k waits for
+    // k - 1 of the same atom, i.e. for the block before this one) relies on blocks being dispatched in index order, which
+    // holds on this hardware but is not a CUDA guarantee; the wait therefore carries the 30 s watchdog and traps rather
+    // than hangs if that ever fails.  Handing out work by an atomicAdd ticket at CTA start makes the order hold by
+    // construction and was measured: cfg 3 19.65 ms against 18.57 ms with the ticket on a cache line of its
+    // own (the cause was not isolated; the placement of neighbouring segments on the SMs changes), so the block index stays.
+    const int seg = blockIdx.x % p.nseg, bg = blockIdx.x / p.nseg;
     const int a = p.seg_atom[seg], qz0 = p.seg_qz0[seg];
     const AtomDev at = p.atoms[a];
     const int Nx = p.g.ng[0], Ny = p.g.ng[1], Nz = p.g.ng[2];
@@ -189,7 +187,7 @@ __global__ void __launch_bounds__(kStoWarps * 32, 2) sho_project_stored_kernel(c
     }
     // ---- the partial sums of the K segments of one (atom, column group) are added to c in segment order: segment k
     // waits until k - 1 has published its sum (a turnstile counter per (atom, group), zeroed by the launcher; the CTA
-    // of segment k - 1 holds the ticket before this one, so it is already running or done), then does a plain
+    // of segment k - 1 has the block index before this one, so it is already running or done), then does a plain
     // read-modify-write.  The wait has the same 30 s watchdog as the mbarrier waits: a lost hand-over traps.  Fixed summation order, no atomics on the data: bit-reproducible.  (fp32 data: each
     // segment's sum is rounded to fp32 when it is added -- the one place where this baseline does not round once.)
     const double h3 = p.g.h * p.g.h * p.g.h;
@@ -289,7 +287,7 @@ sho_status tables_build(const sho_plan* pl, sho_tables** out, size_t* bytes_need
         set_error("sho_tables_build: cudaMalloc of %zu bytes failed", t->bytes);
         return fail(SHO_ERR_OOM);
     }
-    if ((e = cudaMalloc(&t->d_turn, (t->turn_count + 1) * sizeof(int))) != cudaSuccess) return fail(cuda_fail(e, "sho_tables_build: turnstile"));
+    if ((e = cudaMalloc(&t->d_turn, t->turn_count * sizeof(int))) != cudaSuccess) return fail(cuda_fail(e, "sho_tables_build: turnstile"));
     if ((e = cudaEventCreateWithFlags(&t->last_launch, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(e, "sho_tables_build: event"));
     if ((e = up((void**)&t->d_atom_off, off.data(), off.size() * 8)) != cudaSuccess ||
         (e = up((void**)&t->d_seg_atom, seg_atom.data(), seg_atom.size() * 4)) != cudaSuccess ||
@@ -332,7 +330,7 @@ static sho_status launch_t(const sho_plan* pl, const sho_tables* tb, const void*
     }
     const long long nblocks = (long long)tb->nseg * ngroups;
     if (nblocks > 0x7fffffffLL) { set_error("sho_project_stored: grid too large"); return SHO_ERR_UNSUPPORTED; }
-    // The ticket and the turnstile counters are per-launch state that lives in the tables object.  Launches that share
+    // The turnstile counters are per-launch state that lives in the tables object.  Launches that share
     // one tables object -- from any stream, from any host thread -- are therefore chained on the device: each waits
     // for the event recorded behind the one before it (a no-op on the first launch and within one stream), and the
     // host side of the chain is held under the object's mutex.  Without this a second launch's memset could clear
@@ -341,9 +339,9 @@ static sho_status launch_t(const sho_plan* pl, const sho_tables* tb, const void*
     cudaError_t e = cudaStreamWaitEvent(s, tb->last_launch, 0);
     // atoms with an empty box have no segment: their coefficients are the zeros written here
     if (e == cudaSuccess) e = cudaMemsetAsync(coeff, 0, (size_t)pl->g.natoms * nbands * pl->g.nsho * elem_size(pl->dtype), s);
-    if (e == cudaSuccess) e = cudaMemsetAsync(tb->d_turn, 0, ((size_t)pl->g.natoms * ngroups + 1) * sizeof(int), s);
+    if (e == cudaSuccess) e = cudaMemsetAsync(tb->d_turn, 0, (size_t)pl->g.natoms * ngroups * sizeof(int), s);
     if (e != cudaSuccess) return cuda_fail(e, "sho_project_stored: memset");
-    p.ticket = reinterpret_cast<unsigned*>(tb->d_turn); p.turn = tb->d_turn + 1; p.ngroups = ngroups;
+    p.turn = tb->d_turn; p.ngroups = ngroups;
     if (nblocks > 0) {
         sho_project_stored_kernel<MTW, DT><<<(unsigned)nblocks, kStoWarps * 32, 0, s>>>(p);
         if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "launch sho_project_stored_kernel");
@@ -468,7 +466,7 @@ static sho_status launch_add_t(const sho_plan* pl, const sho_tables* tb, const v
     StoParams p;
     p.g = pl->g; p.psi = psi; p.coeff = const_cast<void*>(coeff); p.data = tb->d_data;
     p.atoms = pl->d_atoms; p.atom_off = tb->d_atom_off; p.seg_atom = tb->d_seg_atom; p.seg_qz0 = tb->d_seg_qz0;
-    p.nseg = tb->nseg; p.nbands = nbands; p.turn = nullptr; p.ticket = nullptr; p.ngroups = 0;
+    p.nseg = tb->nseg; p.nbands = nbands; p.turn = nullptr; p.ngroups = 0;
     p.band_stride = (long long)pl->g.ng[0] * pl->g.ng[1] * pl->g.ng[2];
     const int ngroups = (nbands * P + kStoCols - 1) / kStoCols;
     const long long nblocks = (long long)tb->nseg * ngroups;

@@ -65,13 +65,16 @@ def check_project(sho, w, psi, coeff_gpu, tol, pairs=None):
     return float(err.max())
 
 
-def run_case(sho, w, stored=True, tol=None):
-    """boxes, project, add, stored project of one workload against the oracle (full comparison)."""
+def run_case(sho, w, stored=True, tol=None, options=None):
+    """boxes, project, add, stored project of one workload against the oracle (full comparison).  ``options``:
+    sho_plan_set_option knobs to set on the plan first."""
     import torch
     tol = tol or TOL[w.dtype]
     wide = np.complex128 if w.is_complex else np.float64
     plan = sho.plan_for(w)
     try:
+        for key, value in (options or {}).items():
+            plan.set_option(key, value)
         assert np.array_equal(plan.boxes(), _oracle_boxes(w)), "integer box ranges differ from the oracle"
         assert plan.nsho == oracle.nsho(w.numax)
         psi = w.psi()
@@ -276,24 +279,22 @@ def _sample_bands(nb, n=8):
 
 
 @pytest.mark.parametrize("bpc", [2, 3, 8])
-def test_project_band_loop_of_a_cta(sho, bpc, monkeypatch):
+def test_project_band_loop_of_a_cta(sho, bpc):
     """A CTA of sho_project may project several consecutive bands with the tables it sampled once (the launch picks
-    that for many bands of a small grid: the paper's workload).  Forced here on small inputs through the library's
-    test knob: band counts that are and are not multiples of the group, real and complex data, remainder rows."""
-    monkeypatch.setenv("SHO_PROJECT_BANDS_PER_CTA", str(bpc))
+    that for many bands of a small grid: the paper's workload).  Forced here on small inputs through the plan's
+    test knob (sho_plan_set_option): band counts that are and are not multiples of the group, real and complex data, remainder rows."""
     for w in (workloads.make_paper(5, "r64", size="small"), workloads.make(5, size="small"), workloads.make(2, size="small")):
         for nb in (w.nbands, 5):
             w.nbands = nb
-            run_case(sho, w, stored=False)
+            run_case(sho, w, stored=False, options={"project_bands_per_cta": bpc})
     # the grouping changes which CTA computes a band, not how: bit-identical coefficients
     import torch
     w = workloads.make(5, size="small")
     plan = sho.plan_for(w)
     try:
         psi = _dev(w.psi())
-        c_grouped = plan.project(psi).clone()
-        monkeypatch.setenv("SHO_PROJECT_BANDS_PER_CTA", "1")
-        c_single = plan.project(psi)
+        c_grouped = plan.set_option("project_bands_per_cta", bpc).project(psi).clone()
+        c_single = plan.set_option("project_bands_per_cta", 1).project(psi)
         torch.cuda.synchronize()
         assert torch.equal(torch.view_as_real(c_grouped), torch.view_as_real(c_single))
     finally:
@@ -422,14 +423,13 @@ def _atoms_touching(w, boxes, pts):
     return np.nonzero(hit.any(axis=1))[0]
 
 
-def test_apply_host_at_cfg5_full_size_with_the_natural_chunk_rule(sho, monkeypatch):
+def test_apply_host_at_cfg5_full_size_with_the_natural_chunk_rule(sho):
     """sho_apply_host -- the call bench.py's end-to-end number is measured through -- at config 5's full size with the
-    library's own chunk rule (no SHO_HOST_CHUNK_BANDS: one 113 MB band per chunk, 64 chunks through the three-slot
+    library's own chunk rule (no "host_chunk_bands" option: one 113 MB band per chunk, 64 chunks through the three-slot
     ring).  The three steps of PAPER.md:187-190 are recomputed by the oracle for two bands at the points of one
     8 x 64 x 8 block of the grid and of a 4 x 4 x 4 block around the cell corner (every image wraps there, Bloch
     phases on all axes): project_pairs for every atom whose box touches those points, dmul, add_points_bands."""
     import torch
-    monkeypatch.delenv("SHO_HOST_CHUNK_BANDS", raising=False)
     w = workloads.make(5)
     assert w.ng == (192, 192, 192) and w.natoms == 1024 and w.nbands == 64 and w.dtype == "c128"
     plan = sho.plan_for(w)
@@ -623,7 +623,7 @@ def test_add_is_bit_reproducible(sho):
 
 @pytest.mark.parametrize("name", ["cfg2-small", "cfg5-small", "ragged"])
 def test_no_write_outside_the_callers_buffers(sho, name):
-    """compute-sanitizer is closed on this pool (profiles/r2_sanitizer.md), so out-of-bounds WRITES are caught here:
+    """compute-sanitizer is closed on this pool (it cannot attach to a process there), so out-of-bounds WRITES are caught here:
     psi and coeff live inside larger allocations whose guard zones (64 KB on each side, a NaN bit pattern) must come
     back untouched from project, add, the stored-projector project and the fused action; reads outside the buffers
     would hit NaNs and fail the finiteness / parity checks of the other tests."""
@@ -763,13 +763,13 @@ def test_host_buffer_entry_points(sho):
 
 
 @pytest.mark.parametrize("k,chunk", [(3, "2"), (3, "3"), (5, "1"), (5, "2")])
-def test_host_buffer_calls_pipeline_band_chunks(sho, k, chunk, monkeypatch):
+def test_host_buffer_calls_pipeline_band_chunks(sho, k, chunk):
     # the *_host calls copy and compute band chunks on three streams; force several (ragged) chunks
-    monkeypatch.setenv("SHO_HOST_CHUNK_BANDS", chunk)
     w = workloads.make(k, size="small")
     wide = np.complex128 if w.is_complex else np.float64
     plan = sho.plan_for(w)
     try:
+        plan.set_option("host_chunk_bands", int(chunk))
         psi = w.psi()
         c = np.zeros((w.natoms, w.nbands, plan.nsho), dtype=psi.dtype)
         plan.project_host(psi, c)
@@ -840,14 +840,14 @@ def test_dmul_and_apply_match_the_oracle(sho, k, dtype):
 
 
 @pytest.mark.parametrize("chunk", ["1", "2"])
-def test_apply_host_pipelines_band_chunks_through_a_bounded_ring(sho, chunk, monkeypatch):
+def test_apply_host_pipelines_band_chunks_through_a_bounded_ring(sho, chunk):
     # 5 bands in chunks of 1 or 2: more chunks than the three ring slots, so slots are reused
-    monkeypatch.setenv("SHO_HOST_CHUNK_BANDS", chunk)
     rng = np.random.default_rng(9)
     ng = (24, 40, 16)
     w = _custom(ng, (1, 1, 1), rng.uniform(0, 1, (6, 3)) * np.array(ng) * 0.25, rng.uniform(0.3, 0.36, 6), 5, 5, rc=4.0)
     plan = sho.plan_for(w)
     try:
+        plan.set_option("host_chunk_bands", int(chunk))
         Dm = w.dmatrix(plan.nsho)
         psi = w.psi()
         geo = (w.ng, w.h, w.periodic, w.kfrac, w.pos, w.sigma, w.numax)
@@ -948,4 +948,8 @@ def test_wrong_arguments_raise(sho):
         sho.Plan((32, 32, 32), 0.25, (0, 0, 0), w.pos, w.sigma, 16)
     with pytest.raises(sho.ShoError):
         sho.Plan((32, 32, 32), 0.25, (1, 1, 1), w.pos, w.sigma, 3, "r64", kfrac=(0.1, 0, 0))
+    for key, value in (("no_such_option", 1), ("project_bands_per_cta", 9), ("project_bands_per_cta", -1), ("host_chunk_bands", -2)):
+        with pytest.raises(sho.ShoError):
+            plan.set_option(key, value)
+    plan.set_option("project_bands_per_cta", 0).set_option("host_chunk_bands", 0)
     plan.close()
