@@ -20,34 +20,48 @@ namespace {
 
 const double kPi = 3.14159265358979323846264338327950288;
 
-// nodes and weights of the n-point Gauss-Hermite rule (weight exp(-x^2)): Newton's iteration on the orthonormal
-// Hermite recurrence, roots in descending order
+// nodes and weights of the n-point Gauss-Hermite rule (weight exp(-x^2)), Golub-Welsch style: the nodes are the
+// eigenvalues of the Jacobi matrix of the Hermite recurrence (symmetric tridiagonal, zero diagonal, off-diagonal
+// b_k = sqrt(k / 2), k = 1 .. n-1).  Eigenvalue i is bracketed by bisection on the Sturm count (number of eigenvalues
+// below lambda = number of negative pivots of T - lambda I), then polished with Newton steps on the orthonormal
+// polynomial p_n; the weight is the Christoffel number 1 / sum_{k<n} p_k(x_i)^2.  Roots in descending order.
 void gauss_hermite(int n, std::vector<double>& x, std::vector<double>& w)
 {
     x.assign(n, 0.0); w.assign(n, 0.0);
-    const int m = (n + 1) / 2;
-    double z = 0.0;
-    for (int i = 0; i < m; ++i) {
-        if (i == 0) z = std::sqrt(2.0 * n + 1.0) - 1.85575 * std::pow(2.0 * n + 1.0, -1.0 / 6.0);
-        else if (i == 1) z -= 1.14 * std::pow((double)n, 0.426) / z;
-        else if (i == 2) z = 1.86 * z - 0.86 * x[0];
-        else if (i == 3) z = 1.91 * z - 0.91 * x[1];
-        else z = 2.0 * z - x[i - 2];
-        double pp = 1.0;
-        for (int it = 0; it < 100; ++it) {
-            double p1 = std::pow(kPi, -0.25), p2 = 0.0;
-            for (int j = 0; j < n; ++j) {
-                const double p3 = p2;
-                p2 = p1;
-                p1 = z * std::sqrt(2.0 / (j + 1.0)) * p2 - std::sqrt((double)j / (j + 1.0)) * p3;
+    auto below = [n](double lam) {                           // eigenvalues of the Jacobi matrix smaller than lam
+        int count = 0;
+        double q = -lam;
+        for (int k = 1; k <= n; ++k) {
+            if (q < 0.0) ++count;
+            if (k == n) break;
+            if (q == 0.0) q = 1e-300;
+            q = -lam - 0.5 * k / q;
+        }
+        return count;
+    };
+    const double bound = std::sqrt(2.0 * n) + 1.0;           // Gershgorin: |x| <= 2 max b_k
+    for (int i = 0; i < (n + 1) / 2; ++i) {                  // the i-th largest root; the rule is symmetric
+        const int rank = n - 1 - i;                          // ascending position of that root
+        double lo = -bound, hi = bound;
+        for (int it = 0; it < 80; ++it) {
+            const double mid = 0.5 * (lo + hi);
+            if (below(mid) > rank) hi = mid; else lo = mid;
+        }
+        double z = (n % 2 == 1 && i == n / 2) ? 0.0 : 0.5 * (lo + hi);
+        double sum = 0.0;
+        for (int it = 0; it < 3; ++it) {
+            double pm = 0.0, pc = std::pow(kPi, -0.25);      // p_0 .. p_n at z (orthonormal for the weight exp(-x^2))
+            sum = 0.0;
+            for (int k = 0; k < n; ++k) {
+                sum += pc * pc;
+                const double pn = z * std::sqrt(2.0 / (k + 1.0)) * pc - std::sqrt((double)k / (k + 1.0)) * pm;
+                pm = pc; pc = pn;
             }
-            pp = std::sqrt(2.0 * n) * p2;
-            const double z1 = z;
-            z = z1 - p1 / pp;
-            if (std::fabs(z - z1) <= 1e-15 * (1.0 + std::fabs(z))) break;
+            if (z == 0.0) break;
+            z -= pc / (std::sqrt(2.0 * n) * pm);             // p_n' = sqrt(2 n) p_{n-1}
         }
         x[i] = z; x[n - 1 - i] = -z;
-        w[i] = 2.0 / (pp * pp); w[n - 1 - i] = w[i];
+        w[i] = 1.0 / sum; w[n - 1 - i] = w[i];
     }
 }
 
